@@ -1,0 +1,193 @@
+/*
+ * mpcd_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, obviously-correct CPU statement of the MPCD solvent step of
+ * Howard, Panagiotopoulos & Nikoubashman (arXiv 1801.10187), written from
+ * /root/reference/PAPER.md.  Citations are "PAPER.md:<line>" plus the section /
+ * equation / algorithm.  Where the paper is silent the reading is the one in
+ * SURVEY.md section 8(c) (A1..A25, G1..G4) and DESIGN.md "Readings".
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference
+ * legs may load this library.  It shares no code, header, table or constant
+ * generator with the CUDA path (paper_1801_10187_b200/csrc); neither includes
+ * the other.
+ *
+ * Rules kept here so the file can be checked against the paper by eye:
+ *   - one loop per step of the method, in the paper's order; no blocking,
+ *     fusion, threading or reordering;
+ *   - "native" precision (float in the mixed model, double in the fp64 model,
+ *     PAPER.md:84, :195) for positions / velocities / streaming / binning;
+ *     double for every cell sum and for the collision arithmetic
+ *     (Alg. 1 line 5);
+ *   - compiled with -O2 -ffp-contract=off (no FMA contraction, so
+ *     fl(x + fl(v*dt)) is two roundings, reading A7), never -ffast-math.
+ *
+ * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): Philox block function vs
+ * ATen's CPU engine and cuRAND's host path; uniform conversions by exactness;
+ * binning vs exact-rational brute force; cell sums vs numpy bincount and exact
+ * fsum; axis statistics; rotation vs scipy Rotation (handedness), RR^T = I;
+ * per-cell momentum / energy conservation; one-step decorrelation closed forms;
+ * Maxwell-Boltzmann KS test; viscosity 8.7 by transverse-mode
+ * decay; AT conservation / Gaussianity / tag-keying; sort multiset + stability.
+ * parity unpinned: none.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ------------------------------------------------------------------------- *
+ * Counter-based RNG: Philox4x32-10 (the paper uses Saru keyed by (cell index,
+ * timestep, seed); north_star replaces it by Philox4x32-10
+ * with the same keying, reading A24).  Block function as published by Salmon
+ * et al. (ref. [74] of the paper): 10 rounds of two 32x32->64
+ * multiplies, key bumped by the Weyl constants between rounds.
+ * ------------------------------------------------------------------------- */
+void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* Domain tags (4th counter word), reading A24. */
+enum { DOM_SHIFT = 1, DOM_AXIS = 2, DOM_AT = 3, DOM_INITPOS = 4, DOM_INITVEL = 5 };
+
+/* Philox(key = seed, ctr = (index, step_lo, step_hi, domain)), reading A24. */
+static void draw_block(uint64_t seed, uint64_t step, uint32_t index, uint32_t domain, uint32_t out[4])
+{
+    uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint32_t ctr[4] = { index, (uint32_t)step, (uint32_t)(step >> 32), domain };
+    oracle_philox4x32_10(ctr, key, out);
+}
+
+/* 32-bit word -> U in (0,1): (b + 0.5) 2^-32, exact in binary64. */
+double oracle_u01_32(uint32_t b) { return ((double)b + 0.5) * (1.0 / 4294967296.0); }
+
+/* two words -> U in [0,1) with 53 bits: ((lo | hi<<32) >> 11) 2^-53. */
+double oracle_u01_53(uint32_t lo, uint32_t hi)
+{
+    uint64_t w = ((uint64_t)lo | ((uint64_t)hi << 32)) >> 11;
+    return (double)w * (1.0 / 9007199254740992.0);
+}
+
+/* ------------------------------------------------------------------------- *
+ * a2. Random grid shift: one vector per step, each component uniform on
+ * (-a/2, a/2) (PAPER.md:37 "random shift ... of +-a/2", :110; readings A4, A5).
+ * Returned in double; the mixed model rounds it once to float (oracle_bin_f32).
+ * ------------------------------------------------------------------------- */
+void oracle_shift(uint64_t seed, uint64_t step, double a, double s[3])
+{
+    uint32_t b[4];
+    draw_block(seed, step, 0u, DOM_SHIFT, b);
+    for (int d = 0; d < 3; ++d) {
+        double U = oracle_u01_32(b[d]);
+        s[d] = (U - 0.5) * a;
+    }
+}
+
+/* ------------------------------------------------------------------------- *
+ * a5 (axis part). Random unit axis per cell by cylindrical projection from
+ * two uniforms, keyed by (seed, step, global cell index)
+ * (PAPER.md:138), stored in double.  Readings A13, A16.
+ * ------------------------------------------------------------------------- */
+void oracle_axis(uint64_t seed, uint64_t step, int64_t Nc, double *axis3)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int64_t c = 0; c < Nc; ++c) {
+        uint32_t b[4];
+        draw_block(seed, step, (uint32_t)c, DOM_AXIS, b);
+        double U1 = oracle_u01_53(b[0], b[1]);
+        double U2 = oracle_u01_53(b[2], b[3]);
+        double z = 2.0 * U1 - 1.0;
+        double phi = two_pi * U2;
+        double rho = sqrt(1.0 - z * z);
+        axis3[3 * c + 0] = rho * cos(phi);
+        axis3[3 * c + 1] = rho * sin(phi);
+        axis3[3 * c + 2] = z;
+    }
+}
+
+/* ------------------------------------------------------------------------- *
+ * a7 (draw part). Andersen-thermostat random velocities: per particle three
+ * Gaussians of variance kT/m by Box-Muller, RNG keyed by (timestep, particle
+ * tag, seed).  Readings A17, A18.  Always double.
+ * ------------------------------------------------------------------------- */
+void oracle_at_draw(uint64_t seed, uint64_t step, int64_t N, const uint32_t *tag, double sigma, double *dv3)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int64_t i = 0; i < N; ++i) {
+        uint32_t b[4];
+        draw_block(seed, step, tag[i], DOM_AT, b);
+        double U0 = oracle_u01_32(b[0]), U1 = oracle_u01_32(b[1]);
+        double U2 = oracle_u01_32(b[2]), U3 = oracle_u01_32(b[3]);
+        double r01 = sqrt(-2.0 * log(U0));
+        double r23 = sqrt(-2.0 * log(U2));
+        double g0 = r01 * cos(two_pi * U1);
+        double g1 = r01 * sin(two_pi * U1);
+        double g2 = r23 * cos(two_pi * U3);   /* the fourth Gaussian is discarded */
+        dv3[3 * i + 0] = sigma * g0;
+        dv3[3 * i + 1] = sigma * g1;
+        dv3[3 * i + 2] = sigma * g2;
+    }
+}
+
+/* ------------------------------------------------------------------------- *
+ * a8. Sort by cell: the permutation that puts particles in
+ * cell order; stable (reading A20).  perm[k] = old index of the particle that
+ * goes to slot k.
+ * ------------------------------------------------------------------------- */
+void oracle_sort_perm(int64_t N, const int32_t *cell, int64_t Nc, int64_t *perm)
+{
+    int64_t *start = (int64_t *)calloc((size_t)Nc + 1, sizeof(int64_t));
+    for (int64_t i = 0; i < N; ++i) start[cell[i] + 1] += 1;
+    for (int64_t c = 0; c < Nc; ++c) start[c + 1] += start[c];
+    for (int64_t i = 0; i < N; ++i) { perm[start[cell[i]]] = i; start[cell[i]] += 1; }
+    free(start);
+}
+
+/* a4 (count part) + a9 helpers that do not depend on the storage precision. */
+
+/* a9. Net momentum, kinetic energy and pooled temperature from the cell arrays
+ * (PAPER.md:130); pooled estimator kT = sum E_rel / sum 1.5 (N_c - 1) over cells
+ * with N_c >= 2 (reading A11). out = {Px, Py, Pz, KE, kT}. */
+void oracle_thermo(int64_t Nc, double m, const int32_t *count, const double *sumv3, const double *ke,
+                   const double *erel, double out[5])
+{
+    double P[3] = { 0, 0, 0 }, K = 0, E = 0, dof = 0;
+    for (int64_t c = 0; c < Nc; ++c) {
+        for (int d = 0; d < 3; ++d) P[d] += m * sumv3[3 * c + d];
+        K += ke[c];
+        if (count[c] >= 2) { E += erel[c]; dof += 1.5 * (double)(count[c] - 1); }
+    }
+    out[0] = P[0]; out[1] = P[1]; out[2] = P[2]; out[3] = K;
+    out[4] = dof > 0 ? E / dof : 0.0;
+}
+
+/* ------------------------------------------------------------------------- *
+ * Everything that touches particle storage exists once per storage precision.
+ * ------------------------------------------------------------------------- */
+#define REAL float
+#define SUF(name) name##_f32
+#include "mpcd_oracle_steps.inc"
+#undef REAL
+#undef SUF
+
+#define REAL double
+#define SUF(name) name##_f64
+#include "mpcd_oracle_steps.inc"
+#undef REAL
+#undef SUF
