@@ -1,0 +1,201 @@
+/*
+ * mpcd.h -- C ABI of the B200-native MPCD solvent step.
+ *
+ * The method is the multiparticle collision dynamics (MPCD) solvent of Howard,
+ * Panagiotopoulos & Nikoubashman, arXiv 1801.10187.  Citations below are
+ * "PAPER.md:<line>" (the text of the paper under /root/reference) plus the
+ * section / equation / algorithm the line falls in; "A<n>" are the readings
+ * listed in DESIGN.md where the paper is silent.
+ *
+ * One MPCD step (Fig. 1):
+ *     stream (eq. 1) -> random grid shift + bin into cells (sect. 3.4)
+ *       -> [sort by cell, every sort_period steps (sect. 3.8)]
+ *       -> cell properties: count, sum v, kinetic energy in fp64 (sect. 3.5)
+ *       -> collide: SRD (eq. 2, Alg. 1) or Andersen thermostat (eq. 4, sect. 3.7)
+ *
+ * Conventions
+ *   - Every call returns int: 0 = MPCD_OK, negative = error.  Nothing throws,
+ *     aborts or prints across the ABI.  mpcd_last_error() gives a description.
+ *   - A handle is used from one host thread at a time.
+ *   - All device work is enqueued on the handle's CUDA stream and is
+ *     asynchronous, except mpcd_get_* / mpcd_set_state which synchronise that
+ *     stream before returning.
+ *   - "host" / "device" is stated for every pointer.  Particle vectors are
+ *     N x 4 arrays of the NATIVE precision: float in MPCD_MIXED, double in
+ *     MPCD_FP64 ("arrays of four-element floating-point vectors",
+ *     PAPER.md:195 mixed-precision model).  The 4th components are padding (A9).
+ *   - The box is [0, box[d]) per axis, periodic (A1); box[d] = n_d * a with
+ *     integer n_d (A2).  Cell linear index c = ix + nx (iy + ny iz) (A8).
+ *   - There is no CPU fallback: without a CUDA device every call that would
+ *     compute returns MPCD_ECUDA.
+ */
+#ifndef MPCD_H_
+#define MPCD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MPCD_ABI_VERSION 1
+
+/* status codes */
+#define MPCD_OK      0
+#define MPCD_EINVAL (-1)  /* bad argument (NULL handle, N < 1, box not a multiple of a, ...) */
+#define MPCD_ENOMEM (-2)  /* the allocator (callback or cudaMalloc) failed */
+#define MPCD_ECUDA  (-3)  /* a CUDA runtime call or kernel launch failed / no device */
+#define MPCD_ESTATE (-4)  /* call not valid in the current state (e.g. collide without a bin) */
+
+/* precision models */
+#define MPCD_MIXED 0      /* fp32 particle data, fp64 cell sums and collision arithmetic */
+#define MPCD_FP64  1      /* everything double */
+
+/* collision rules */
+#define MPCD_SRD 0        /* stochastic rotation dynamics, eq. 2 */
+#define MPCD_AT  1        /* Andersen thermostat, eq. 4 */
+
+typedef struct mpcd mpcd_t;   /* opaque */
+
+/* Device-memory callbacks: PyTorch (or any caller) supplies every O(N) and
+ * O(N_cells) buffer through these; `bytes` is a multiple of 256 and the returned
+ * DEVICE pointer must be 256-byte aligned and stay valid until free_fn is called
+ * with it.  alloc_fn returns NULL on failure.  When both are NULL the library
+ * uses cudaMalloc / cudaFree. */
+typedef void *(*mpcd_alloc_fn)(size_t bytes, void *user);
+typedef void (*mpcd_free_fn)(void *device_ptr, void *user);
+
+typedef struct mpcd_options {
+    int32_t precision;     /* MPCD_MIXED (default) | MPCD_FP64 */
+    int32_t rule;          /* MPCD_SRD (default) | MPCD_AT: the rule mpcd_step applies */
+    double dt;             /* collision time, default 0.1 */
+    double alpha;          /* SRD angle in radians (A15), default 130 deg */
+    int32_t sort_period;   /* sort every k steps, t % k == 0 (A21); 0 = never; default 25 */
+    int32_t cell_energy;   /* 1 (default): accumulate the per-cell kinetic energy every step (sect. 3.5);
+                              0: momentum and count only (KE is then computed on demand by mpcd_get_cells / thermo) */
+    int32_t init_state;    /* 1 (default): draw the initial condition on the device (A23); 0: leave the particle
+                              arrays uninitialised, the caller must mpcd_set_state before stepping */
+    int32_t reserved0;
+    void *stream;          /* cudaStream_t the library enqueues on; NULL = the legacy default stream */
+    mpcd_alloc_fn alloc_fn;
+    mpcd_free_fn free_fn;
+    void *alloc_user;
+} mpcd_options;
+
+/* Fills *opt with the defaults above.  opt: host. */
+int mpcd_default_options(mpcd_options *opt);
+
+/*
+ * mpcd_create -- allocate a solvent of N particles of mass m in a periodic box
+ * `box` (host, 3 doubles) of cubic collision cells of edge a, at
+ * temperature kT, with RNG seed `seed` ("user-supplied seed").
+ * Errors: MPCD_EINVAL if out == NULL, N < 1, N >= 2^31, a, m, kT <= 0, box[d]
+ * not an integer multiple of a (|box/a - n_d| <= 1e-9) or n_x n_y n_z >= 2^31;
+ * MPCD_ENOMEM / MPCD_ECUDA on allocation / device failure (then *out = NULL).
+ * Initial state (A23): positions uniform in the box, velocities N(0, kT/m) with
+ * the mean removed, tags 0..N-1, step counter 0.
+ * The handle is owned by the caller until mpcd_destroy.
+ */
+int mpcd_create(mpcd_t **out, const double box[3], int64_t N, double a, double m, double kT, uint64_t seed);
+int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, double m, double kT, uint64_t seed,
+                   const mpcd_options *opt /* host, may be NULL */);
+int mpcd_destroy(mpcd_t *h);
+
+/* a1. Streaming, eq. 1: r <- r + v dt in native precision (two
+ * roundings, no FMA, A7), wrapped into [0, L).  Invalidates the current bin. */
+int mpcd_stream(mpcd_t *h);
+
+/* a2-a5. For the current step counter t: draw the grid shift from
+ * Philox(seed, t) (A4, A5), bin every particle with the shift
+ * applied during binning only (A6), accumulate per cell the count,
+ * sum of velocities and kinetic energy in fp64, then per cell
+ * the mean velocity u, the relative kinetic energy / temperature (eq. 3
+ * PAPER.md:47; A11) and the random unit axis from Philox(seed, t, cell) by
+ * cylindrical projection (A13).  Idempotent for a given
+ * (state, t).  Direct fp64 accumulation has no capacity, so the overflow /
+ * rebuild path of PAPER.md:110 does not exist. */
+int mpcd_shift_and_bin(mpcd_t *h);
+
+/* a6. SRD collision, eq. 2 / Algorithm 1, angle alpha in
+ * radians about each cell's axis, fp64 arithmetic, native-precision store.
+ * Needs a valid bin for the current step (else MPCD_ESTATE).  Does not advance
+ * the step counter.  Invalidates the cell sums (velocities changed). */
+int mpcd_collide_srd(mpcd_t *h, double alpha);
+
+/* a7. Andersen-thermostat collision, eq. 4, sect. 3.7 PAPER.md:163:
+ * per-particle Gaussians from Philox(seed, t, tag) by Box-Muller (A17, A18), a
+ * second per-cell reduction, v <- u + dv - sum(dv)/N_c.  Same preconditions. */
+int mpcd_collide_at(mpcd_t *h);
+
+/* a8. Sort by cell, sect. 3.8: reorder pos, vel, tag and cell
+ * into ascending cell order using the current bin (MPCD_ESTATE if none).  Order
+ * within a cell is unspecified (A20).  Tags travel with particles. */
+int mpcd_sort(mpcd_t *h);
+
+/* nsteps x { stream; shift_and_bin; sort if sort_period and t % sort_period == 0;
+ * collide per opt.rule; t += 1 } (A3).  Internally the collision of
+ * step t is fused with the streaming / binning / accumulation of step t + 1
+ * (one pass over the particles per step); the result is the same as the unfused
+ * sequence of calls up to fp64 summation order. */
+int mpcd_step(mpcd_t *h, int32_t nsteps);
+
+/* Copies the particle state to caller-owned HOST buffers (any may be NULL):
+ * pos4 / vel4 = N x 4 native precision, tag = N x u32, cell = N x i32 (last bin;
+ * unspecified if none), step = the step counter.  Order is the current (possibly
+ * sorted) order: compare by tag.  Synchronises the stream. */
+int mpcd_get_state(mpcd_t *h, void *pos4, void *vel4, uint32_t *tag, int32_t *cell, uint64_t *step);
+
+/* Overwrites the particle state from HOST buffers (pos4, vel4 required, N x 4
+ * native precision; tag may be NULL = 0..N-1) and sets the step counter.
+ * Positions must lie in [0, box).  Invalidates the bin.  Synchronises. */
+int mpcd_set_state(mpcd_t *h, const void *pos4, const void *vel4, const uint32_t *tag, uint64_t step);
+
+/* Per-cell results of the last mpcd_shift_and_bin to HOST buffers (any may be
+ * NULL): count[Nc] i32, sumv3[Nc*3], ke[Nc], u3[Nc*3], axis3[Nc*3], kTc[Nc],
+ * all double.  MPCD_ESTATE if the cell sums are not valid (no bin, or a
+ * collision has changed the velocities since). */
+int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double *u3, double *axis3, double *kTc);
+
+/* The shift used by the last bin, as applied (mixed mode: the fp32 value, A5).  s: host. */
+int mpcd_get_shift(mpcd_t *h, double s[3]);
+
+/* a9. Net momentum P (3), kinetic energy and pooled temperature (A11) of the
+ * CURRENT velocities by device-wide reduction.  If no bin is valid
+ * one is made for the current step.  Outputs: host, any may be NULL. */
+int mpcd_get_thermo(mpcd_t *h, double P[3], double *KE, double *kT);
+
+typedef struct mpcd_stats {
+    int64_t N;              /* particles */
+    int64_t Nc;             /* cells */
+    int32_t n[3];           /* cells per axis */
+    int32_t max_occupancy;  /* largest cell count seen in the last bin */
+    uint64_t step;          /* step counter */
+    uint64_t kernel_launches; /* kernels launched by this handle so far */
+    uint64_t sorts;         /* sorts done so far */
+    uint64_t device_bytes;  /* bytes obtained from the allocator */
+} mpcd_stats;
+int mpcd_get_stats(mpcd_t *h, mpcd_stats *out /* host */);
+
+/* DEVICE pointers of the current particle arrays (for zero-copy inspection; they
+ * change after a sort).  Any output may be NULL. */
+int mpcd_device_ptrs(mpcd_t *h, void **pos4, void **vel4, uint32_t **tag, int32_t **cell);
+
+/* Static description of the last error on this handle (or of the last failed
+ * mpcd_create when h == NULL).  Never NULL. */
+const char *mpcd_last_error(const mpcd_t *h);
+
+/* Library identification: ABI version; build string (arch, compiler). */
+int mpcd_abi_version(void);
+const char *mpcd_build_info(void);
+
+/* Test hook: the library's own Philox4x32-10 block function evaluated ON THE
+ * DEVICE for n (ctr, key) pairs; ctr4: host n x 4 u32, key2: host n x 2 u32,
+ * out4: host n x 4 u32.  Used to pin the CUDA generator against the oracle and
+ * cuRAND. */
+int mpcd_test_philox(const uint32_t *ctr4, const uint32_t *key2, uint32_t *out4, int64_t n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPCD_H_ */

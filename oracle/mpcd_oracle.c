@@ -114,7 +114,7 @@ void oracle_axis(uint64_t seed, uint64_t step, int64_t Nc, double *axis3)
         double U2 = oracle_u01_53(b[2], b[3]);
         double z = 2.0 * U1 - 1.0;
         double phi = two_pi * U2;
-        double rho = sqrt(1.0 - z * z);
+        double rho = sqrt((1.0 - z) * (1.0 + z));   /* = sqrt(1 - z^2) without the cancellation near the poles */
         axis3[3 * c + 0] = rho * cos(phi);
         axis3[3 * c + 1] = rho * sin(phi);
         axis3[3 * c + 2] = z;

@@ -1,0 +1,662 @@
+// mpcd.cu -- host side of the C ABI declared in include/mpcd.h: handle, memory, the step
+// scheduler and the kernel launches.  All arithmetic of the method runs in the kernels of
+// mpcd_kernels.cuh; the only method arithmetic on the host is the three-scalar grid-shift
+// draw (a2) and cos/sin of the SRD angle (A15).
+#include "../../include/mpcd.h"
+#include "mpcd_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace mpcdk;
+
+namespace {
+
+thread_local char g_create_error[256] = "no error";
+
+struct Buffer { void *ptr; size_t bytes; };
+
+}  // namespace
+
+struct mpcd {
+    // parameters
+    int64_t N = 0, Nc = 0;
+    int32_t n[3] = {0, 0, 0};
+    double box[3] = {0, 0, 0};
+    double a = 1, m = 1, kT = 1, sigma = 1;
+    uint64_t seed = 0;
+    mpcd_options opt{};
+    cudaStream_t stream = nullptr;
+    // particle arrays, double-buffered for the sort
+    void *pos[2] = {nullptr, nullptr}, *vel[2] = {nullptr, nullptr};
+    uint32_t *tag[2] = {nullptr, nullptr};
+    int32_t *cell[2] = {nullptr, nullptr};
+    int pcur = 0;
+    // cell arrays
+    double *acc[2] = {nullptr, nullptr};
+    int32_t *cnt[2] = {nullptr, nullptr};
+    double *at_acc[2] = {nullptr, nullptr};
+    CellRec *rec = nullptr;
+    int32_t *cell_start = nullptr, *tile_sum = nullptr;
+    int *d_max_occ = nullptr;
+    double *d_scalars = nullptr;   // 8 doubles of scratch for reductions
+    int ccur = 0;                  // accumulator set of the current bin
+    bool zeroed[2] = {false, false}, at_zeroed[2] = {false, false};
+    // state machine
+    uint64_t step = 0, bin_step = 0;
+    bool bin_valid = false, sums_valid = false, energy_valid = false, rec_valid = false;
+    int rec_mode = 0;
+    double shift_used[3] = {0, 0, 0};
+    // bookkeeping
+    std::vector<Buffer> buffers;
+    uint64_t launches = 0, sorts = 0, device_bytes = 0;
+    char err[256] = "no error";
+};
+
+namespace {
+
+int fail(mpcd_t *h, int code, const char *fmt, const char *detail = "")
+{
+    char *dst = h ? h->err : g_create_error;
+    snprintf(dst, 256, fmt, detail);
+    return code;
+}
+
+#define CUDA_TRY(h, expr)                                                        \
+    do {                                                                         \
+        cudaError_t e_ = (expr);                                                 \
+        if (e_ != cudaSuccess) return fail((h), MPCD_ECUDA, #expr ": %s", cudaGetErrorString(e_)); \
+    } while (0)
+
+#define LAUNCH_CHECK(h)                                                          \
+    do {                                                                         \
+        (h)->launches += 1;                                                      \
+        cudaError_t e_ = cudaGetLastError();                                     \
+        if (e_ != cudaSuccess) return fail((h), MPCD_ECUDA, "kernel launch: %s", cudaGetErrorString(e_)); \
+    } while (0)
+
+int dev_alloc(mpcd_t *h, void **out, size_t bytes)
+{
+    bytes = (bytes + 255) & ~(size_t)255;
+    if (bytes == 0) bytes = 256;
+    void *p = nullptr;
+    if (h->opt.alloc_fn) {
+        p = h->opt.alloc_fn(bytes, h->opt.alloc_user);
+        if (!p) return fail(h, MPCD_ENOMEM, "allocator callback returned NULL%s");
+    } else {
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(h, MPCD_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
+    }
+    h->buffers.push_back(Buffer{p, bytes});
+    h->device_bytes += bytes;
+    *out = p;
+    return MPCD_OK;
+}
+
+template <typename P> int dev_alloc_t(mpcd_t *h, P **out, size_t count) { return dev_alloc(h, reinterpret_cast<void **>(out), count * sizeof(P)); }
+
+inline size_t native_size(const mpcd_t *h) { return h->opt.precision == MPCD_FP64 ? sizeof(double) : sizeof(float); }
+inline unsigned grid_for(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+// a2: the step's grid shift, uniform on (-a/2, a/2)^3 from Philox(seed, (0, t, SHIFT)) (A4, A5)
+void draw_shift(const mpcd_t *h, uint64_t step, double s[3])
+{
+    const u32x4 b = draw(h->seed, step, 0u, kDomShift);
+    const uint32_t w[3] = {b.x, b.y, b.z};
+    for (int d = 0; d < 3; ++d) s[d] = (u01_32(w[d]) - 0.5) * h->a;
+}
+
+template <typename T> PassArgs<T> make_args(mpcd_t *h, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
+{
+    PassArgs<T> a{};
+    a.pos = static_cast<typename Vec4<T>::type *>(h->pos[h->pcur]);
+    a.vel = static_cast<typename Vec4<T>::type *>(h->vel[h->pcur]);
+    a.tag = h->tag[h->pcur];
+    a.cell = h->cell[h->pcur];
+    a.rec = h->rec;
+    a.acc = h->acc[acc_set];
+    a.cnt = h->cnt[acc_set];
+    a.at_acc = h->at_acc[acc_set];
+    a.N = h->N;
+    for (int d = 0; d < 3; ++d) {
+        a.n[d] = h->n[d];
+        a.L[d] = (T)h->box[d];
+        a.shift[d] = (T)shift[d];
+    }
+    a.dt = (T)h->opt.dt;
+    a.inv_a = (T)1 / (T)h->a;
+    a.cos_a = std::cos(alpha);
+    a.sin_a = std::sin(alpha);
+    a.sigma = h->sigma;
+    a.seed = h->seed;
+    a.step_collide = step_collide;
+    a.step_bin = step_bin;
+    return a;
+}
+
+template <typename T, unsigned F> void launch_pass_t(mpcd_t *h, const PassArgs<T> &a)
+{
+    particle_pass<T, F><<<grid_for(h->N, kPassThreads), kPassThreads, 0, h->stream>>>(a);
+}
+
+template <typename T> int launch_pass(mpcd_t *h, unsigned F, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
+{
+    const PassArgs<T> a = make_args<T>(h, acc_set, step_collide, step_bin, shift, alpha);
+    switch (F) {
+#define CASE(f) case (f): launch_pass_t<T, (f)>(h, a); break;
+        CASE(kStream)
+        CASE(kBin)
+        CASE(kBin | kEnergy)
+        CASE(kStream | kBin)
+        CASE(kStream | kBin | kEnergy)
+        CASE(kStream | kBin | kATDraw)
+        CASE(kStream | kBin | kATDraw | kEnergy)
+        CASE(kSRD)
+        CASE(kSRD | kStream | kBin)
+        CASE(kSRD | kStream | kBin | kEnergy)
+        CASE(kATDraw)
+        CASE(kATApply)
+        CASE(kATApply | kStream | kBin | kATDraw)
+        CASE(kATApply | kStream | kBin | kATDraw | kEnergy)
+#undef CASE
+        default: return fail(h, MPCD_EINVAL, "internal: pass combination not instantiated%s");
+    }
+    LAUNCH_CHECK(h);
+    return MPCD_OK;
+}
+
+int pass(mpcd_t *h, unsigned F, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
+{
+    return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, acc_set, step_collide, step_bin, shift, alpha)
+                                         : launch_pass<float>(h, F, acc_set, step_collide, step_bin, shift, alpha);
+}
+
+int ensure_at_buffers(mpcd_t *h)
+{
+    if (h->at_acc[0]) return MPCD_OK;
+    for (int s = 0; s < 2; ++s) {
+        int rc = dev_alloc_t(h, &h->at_acc[s], (size_t)h->Nc * 4);
+        if (rc) return rc;
+        h->at_zeroed[s] = false;
+    }
+    return MPCD_OK;
+}
+
+int zero_set(mpcd_t *h, int s, bool sums, bool at)
+{
+    sums = sums && !h->zeroed[s];
+    at = at && h->at_acc[s] && !h->at_zeroed[s];
+    if (!sums && !at) return MPCD_OK;
+    cell_zero<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(sums ? h->acc[s] : nullptr, h->cnt[s], at ? h->at_acc[s] : nullptr, h->Nc);
+    LAUNCH_CHECK(h);
+    if (sums) h->zeroed[s] = true;
+    if (at) h->at_zeroed[s] = true;
+    return MPCD_OK;
+}
+
+// a5 for accumulator set `s` at step `t`; optionally zero the other set for the next step.
+int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool zero_next)
+{
+    FinalizeArgs f{};
+    f.acc = h->acc[s]; f.cnt = h->cnt[s]; f.at_acc = h->at_acc[s];
+    const int o = s ^ 1;
+    const bool zs = zero_next && !h->zeroed[o];
+    const bool za = zero_next && h->at_acc[o] && !h->at_zeroed[o] && at_mode;
+    f.acc_next = zs ? h->acc[o] : nullptr;
+    f.cnt_next = zs ? h->cnt[o] : nullptr;
+    f.at_acc_next = za ? h->at_acc[o] : nullptr;
+    f.rec = h->rec;
+    f.max_occupancy = h->d_max_occ;
+    f.Nc = h->Nc; f.m = h->m; f.seed = h->seed; f.step = t;
+    f.at_mode = at_mode; f.have_energy = have_energy ? 1 : 0;
+    CUDA_TRY(h, cudaMemsetAsync(h->d_max_occ, 0, sizeof(int), h->stream));
+    cell_finalize<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(f);
+    LAUNCH_CHECK(h);
+    if (zs) h->zeroed[o] = true;
+    if (za) h->at_zeroed[o] = true;
+    h->rec_valid = true;
+    h->rec_mode = at_mode;
+    return MPCD_OK;
+}
+
+// a8: counting sort by cell on the counts of accumulator set `s`.
+int do_sort(mpcd_t *h, int s)
+{
+    const int ntiles = (int)((h->Nc + kScanTile - 1) / kScanTile);
+    scan_tile_sums<<<ntiles, kScanThreads, 0, h->stream>>>(h->cnt[s], h->Nc, h->tile_sum);
+    LAUNCH_CHECK(h);
+    scan_tile_offsets<<<1, 1024, 0, h->stream>>>(h->tile_sum, ntiles);
+    LAUNCH_CHECK(h);
+    scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->cnt[s], h->Nc, h->tile_sum, h->cell_start);
+    LAUNCH_CHECK(h);
+    const int src = h->pcur, dst = src ^ 1;
+    if (h->opt.precision == MPCD_FP64)
+        sort_scatter<double><<<grid_for(h->N, 256), 256, 0, h->stream>>>(h->N, (const double4 *)h->pos[src], (const double4 *)h->vel[src], h->tag[src],
+                                                                     h->cell[src], h->cell_start, (double4 *)h->pos[dst], (double4 *)h->vel[dst],
+                                                                     h->tag[dst], h->cell[dst]);
+    else
+        sort_scatter<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(h->N, (const float4 *)h->pos[src], (const float4 *)h->vel[src], h->tag[src],
+                                                                    h->cell[src], h->cell_start, (float4 *)h->pos[dst], (float4 *)h->vel[dst],
+                                                                    h->tag[dst], h->cell[dst]);
+    LAUNCH_CHECK(h);
+    h->pcur = dst;
+    h->sorts += 1;
+    return MPCD_OK;
+}
+
+inline bool sort_due(const mpcd_t *h, uint64_t t) { return h->opt.sort_period > 0 && (t % (uint64_t)h->opt.sort_period) == 0; }
+
+// bin + accumulate (+ finalize) for step t as a standalone block; energy always accumulated here
+int bin_accumulate(mpcd_t *h, uint64_t t, bool with_stream)
+{
+    double s[3];
+    draw_shift(h, t, s);
+    if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) s[d] = (double)(float)s[d];   // A5
+    const int set = h->ccur;
+    int rc = zero_set(h, set, true, false);
+    if (rc) return rc;
+    h->zeroed[set] = false;
+    rc = pass(h, (with_stream ? kStream : 0u) | kBin | kEnergy, set, t, t, s, h->opt.alpha);
+    if (rc) return rc;
+    for (int d = 0; d < 3; ++d) h->shift_used[d] = s[d];
+    h->bin_valid = true; h->bin_step = t;
+    rc = finalize(h, set, t, 0, true, false);
+    if (rc) return rc;
+    h->sums_valid = true; h->energy_valid = true;
+    return MPCD_OK;
+}
+
+int init_state(mpcd_t *h)
+{
+    CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, 8 * sizeof(double), h->stream));
+    const unsigned g = grid_for(h->N, 256);
+    if (h->opt.precision == MPCD_FP64)
+        init_particles<double><<<g, 256, 0, h->stream>>>(h->N, h->seed, h->box[0], h->box[1], h->box[2], h->sigma, nullptr, h->d_scalars,
+                                                       (double4 *)h->pos[0], (double4 *)h->vel[0], h->tag[0]);
+    else
+        init_particles<float><<<g, 256, 0, h->stream>>>(h->N, h->seed, h->box[0], h->box[1], h->box[2], h->sigma, nullptr, h->d_scalars,
+                                                      (float4 *)h->pos[0], (float4 *)h->vel[0], h->tag[0]);
+    LAUNCH_CHECK(h);
+    double sum[3];
+    CUDA_TRY(h, cudaMemcpyAsync(sum, h->d_scalars, 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    double mean[3] = {sum[0] / (double)h->N, sum[1] / (double)h->N, sum[2] / (double)h->N};
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_scalars + 4, mean, 3 * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    if (h->opt.precision == MPCD_FP64)
+        init_particles<double><<<g, 256, 0, h->stream>>>(h->N, h->seed, h->box[0], h->box[1], h->box[2], h->sigma, h->d_scalars + 4, nullptr,
+                                                       (double4 *)h->pos[0], (double4 *)h->vel[0], h->tag[0]);
+    else
+        init_particles<float><<<g, 256, 0, h->stream>>>(h->N, h->seed, h->box[0], h->box[1], h->box[2], h->sigma, h->d_scalars + 4, nullptr,
+                                                      (float4 *)h->pos[0], (float4 *)h->vel[0], h->tag[0]);
+    LAUNCH_CHECK(h);
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return MPCD_OK;
+}
+
+void release(mpcd_t *h)
+{
+    for (const Buffer &b : h->buffers) {
+        if (h->opt.free_fn) h->opt.free_fn(b.ptr, h->opt.alloc_user);
+        else if (!h->opt.alloc_fn) cudaFree(b.ptr);
+    }
+    h->buffers.clear();
+}
+
+}  // namespace
+
+// =========================================================================================
+// C ABI
+// =========================================================================================
+extern "C" {
+
+int mpcd_default_options(mpcd_options *opt)
+{
+    if (!opt) return MPCD_EINVAL;
+    std::memset(opt, 0, sizeof(*opt));
+    opt->precision = MPCD_MIXED;
+    opt->rule = MPCD_SRD;
+    opt->dt = 0.1;
+    opt->alpha = 130.0 * 3.14159265358979323846 / 180.0;
+    opt->sort_period = 25;
+    opt->cell_energy = 1;
+    opt->init_state = 1;
+    return MPCD_OK;
+}
+
+int mpcd_create(mpcd_t **out, const double box[3], int64_t N, double a, double m, double kT, uint64_t seed)
+{
+    return mpcd_create_ex(out, box, N, a, m, kT, seed, nullptr);
+}
+
+int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, double m, double kT, uint64_t seed, const mpcd_options *opt)
+{
+    if (!out) return fail(nullptr, MPCD_EINVAL, "out is NULL%s");
+    *out = nullptr;
+    if (!box) return fail(nullptr, MPCD_EINVAL, "box is NULL%s");
+    if (N < 1 || N >= ((int64_t)1 << 31)) return fail(nullptr, MPCD_EINVAL, "N must be in [1, 2^31)%s");
+    if (!(a > 0) || !(m > 0) || !(kT > 0)) return fail(nullptr, MPCD_EINVAL, "a, m, kT must be positive%s");
+    mpcd_options o;
+    mpcd_default_options(&o);
+    if (opt) o = *opt;
+    if (o.precision != MPCD_MIXED && o.precision != MPCD_FP64) return fail(nullptr, MPCD_EINVAL, "bad precision%s");
+    if (o.rule != MPCD_SRD && o.rule != MPCD_AT) return fail(nullptr, MPCD_EINVAL, "bad rule%s");
+    if (!(o.dt > 0) || o.sort_period < 0) return fail(nullptr, MPCD_EINVAL, "dt must be > 0 and sort_period >= 0%s");
+    if ((o.alloc_fn == nullptr) != (o.free_fn == nullptr)) return fail(nullptr, MPCD_EINVAL, "alloc_fn and free_fn must be given together%s");
+    int32_t n[3];
+    double ncells = 1;
+    for (int d = 0; d < 3; ++d) {
+        const double q = box[d] / a;
+        const double r = std::floor(q + 0.5);
+        if (!(r >= 1) || std::fabs(q - r) > 1e-9 || r >= 2147483648.0) return fail(nullptr, MPCD_EINVAL, "box must be a positive integer multiple of a%s");
+        n[d] = (int32_t)r;
+        ncells *= r;
+    }
+    if (ncells >= 2147483648.0) return fail(nullptr, MPCD_EINVAL, "number of cells must be < 2^31%s");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, MPCD_ECUDA, "no CUDA device: this library has no CPU fallback%s");
+    }
+    mpcd_t *h = new (std::nothrow) mpcd();
+    if (!h) return fail(nullptr, MPCD_ENOMEM, "host allocation failed%s");
+    h->N = N; h->a = a; h->m = m; h->kT = kT; h->sigma = std::sqrt(kT / m); h->seed = seed; h->opt = o;
+    h->stream = static_cast<cudaStream_t>(o.stream);
+    for (int d = 0; d < 3; ++d) { h->n[d] = n[d]; h->box[d] = box[d]; }
+    h->Nc = (int64_t)n[0] * n[1] * n[2];
+    const size_t ns = native_size(h);
+    int rc = MPCD_OK;
+    for (int s = 0; s < 2 && !rc; ++s) {
+        rc = dev_alloc(h, &h->pos[s], (size_t)N * 4 * ns);
+        if (!rc) rc = dev_alloc(h, &h->vel[s], (size_t)N * 4 * ns);
+        if (!rc) rc = dev_alloc_t(h, &h->tag[s], (size_t)N);
+        if (!rc) rc = dev_alloc_t(h, &h->cell[s], (size_t)N);
+        if (!rc) rc = dev_alloc_t(h, &h->acc[s], (size_t)h->Nc * 4);
+        if (!rc) rc = dev_alloc_t(h, &h->cnt[s], (size_t)h->Nc);
+    }
+    if (!rc) rc = dev_alloc_t(h, &h->rec, (size_t)h->Nc);
+    if (!rc) rc = dev_alloc_t(h, &h->cell_start, (size_t)h->Nc + 1);
+    if (!rc) rc = dev_alloc_t(h, &h->tile_sum, (size_t)((h->Nc + kScanTile - 1) / kScanTile) + 1);
+    if (!rc) rc = dev_alloc_t(h, &h->d_max_occ, 64);
+    if (!rc) rc = dev_alloc_t(h, &h->d_scalars, 32);
+    if (!rc && o.rule == MPCD_AT) rc = ensure_at_buffers(h);
+    if (!rc && cudaMemsetAsync(h->cell[0], 0, (size_t)N * sizeof(int32_t), h->stream) != cudaSuccess) rc = fail(h, MPCD_ECUDA, "memset failed%s");
+    if (!rc && o.init_state) rc = init_state(h);
+    if (rc) {
+        std::memcpy(g_create_error, h->err, sizeof(g_create_error));
+        release(h);
+        delete h;
+        return rc;
+    }
+    *out = h;
+    return MPCD_OK;
+}
+
+int mpcd_destroy(mpcd_t *h)
+{
+    if (!h) return MPCD_EINVAL;
+    cudaStreamSynchronize(h->stream);
+    release(h);
+    delete h;
+    return MPCD_OK;
+}
+
+int mpcd_stream(mpcd_t *h)
+{
+    if (!h) return MPCD_EINVAL;
+    const double zero[3] = {0, 0, 0};
+    int rc = pass(h, kStream, h->ccur, h->step, h->step, zero, h->opt.alpha);
+    if (rc) return rc;
+    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    return MPCD_OK;
+}
+
+int mpcd_shift_and_bin(mpcd_t *h)
+{
+    if (!h) return MPCD_EINVAL;
+    return bin_accumulate(h, h->step, false);
+}
+
+int mpcd_collide_srd(mpcd_t *h, double alpha)
+{
+    if (!h) return MPCD_EINVAL;
+    if (!(h->bin_valid && h->bin_step == h->step && h->sums_valid && h->rec_valid))
+        return fail(h, MPCD_ESTATE, "collide_srd needs mpcd_shift_and_bin for the current step first%s");
+    if (h->rec_mode != 0) {
+        int rc = finalize(h, h->ccur, h->step, 0, h->energy_valid, false);
+        if (rc) return rc;
+    }
+    int rc = pass(h, kSRD, h->ccur, h->step, h->step, h->shift_used, alpha);
+    if (rc) return rc;
+    h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    return MPCD_OK;
+}
+
+int mpcd_collide_at(mpcd_t *h)
+{
+    if (!h) return MPCD_EINVAL;
+    if (!(h->bin_valid && h->bin_step == h->step && h->sums_valid))
+        return fail(h, MPCD_ESTATE, "collide_at needs mpcd_shift_and_bin for the current step first%s");
+    int rc = ensure_at_buffers(h);
+    if (rc) return rc;
+    const int set = h->ccur;
+    rc = zero_set(h, set, false, true);
+    if (rc) return rc;
+    h->at_zeroed[set] = false;
+    rc = pass(h, kATDraw, set, h->step, h->step, h->shift_used, h->opt.alpha);       // second reduction
+    if (!rc) rc = finalize(h, set, h->step, 1, h->energy_valid, false);
+    if (!rc) rc = pass(h, kATApply, set, h->step, h->step, h->shift_used, h->opt.alpha);
+    if (rc) return rc;
+    h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    return MPCD_OK;
+}
+
+int mpcd_sort(mpcd_t *h)
+{
+    if (!h) return MPCD_EINVAL;
+    if (!(h->bin_valid && h->sums_valid)) return fail(h, MPCD_ESTATE, "sort needs a valid bin (mpcd_shift_and_bin)%s");
+    return do_sort(h, h->ccur);
+}
+
+int mpcd_step(mpcd_t *h, int32_t nsteps)
+{
+    if (!h) return MPCD_EINVAL;
+    if (nsteps < 0) return fail(h, MPCD_EINVAL, "nsteps must be >= 0%s");
+    if (nsteps == 0) return MPCD_OK;
+    const bool at = h->opt.rule == MPCD_AT;
+    const bool energy = h->opt.cell_energy != 0;
+    const unsigned fe = energy ? kEnergy : 0u;
+    int rc = at ? ensure_at_buffers(h) : MPCD_OK;
+    if (rc) return rc;
+    const double alpha = h->opt.alpha;
+    uint64_t t = h->step;
+    double s[3];
+    auto shift_for = [&](uint64_t step) {
+        draw_shift(h, step, s);
+        if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) s[d] = (double)(float)s[d];
+    };
+    // first block: stream + bin + accumulate for step t
+    int set = h->ccur;
+    rc = zero_set(h, set, true, at);
+    if (rc) return rc;
+    shift_for(t);
+    h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
+    rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), set, t, t, s, alpha);
+    if (rc) return rc;
+    if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
+    rc = finalize(h, set, t, at ? 1 : 0, energy, nsteps > 1);
+    if (rc) return rc;
+    // steady state: collide(t) fused with stream + bin + accumulate (t + 1): one pass per step
+    for (int32_t j = 1; j < nsteps; ++j) {
+        const int nxt = set ^ 1;
+        rc = zero_set(h, nxt, true, at);            // no-op when finalize already zeroed it
+        if (rc) return rc;
+        shift_for(t + 1);
+        h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
+        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe, nxt, t, t + 1, s, alpha);
+        if (rc) return rc;
+        set = nxt; t += 1;
+        if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
+        rc = finalize(h, set, t, at ? 1 : 0, energy, j + 1 < nsteps);
+        if (rc) return rc;
+    }
+    // last collision
+    rc = pass(h, at ? kATApply : kSRD, set, t, t, s, alpha);
+    if (rc) return rc;
+    h->ccur = set;
+    for (int d = 0; d < 3; ++d) h->shift_used[d] = s[d];
+    h->bin_valid = true; h->bin_step = t;
+    h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    h->step = t + 1;
+    return MPCD_OK;
+}
+
+int mpcd_get_state(mpcd_t *h, void *pos4, void *vel4, uint32_t *tag, int32_t *cell, uint64_t *step)
+{
+    if (!h) return MPCD_EINVAL;
+    const size_t vb = (size_t)h->N * 4 * native_size(h);
+    if (pos4) CUDA_TRY(h, cudaMemcpyAsync(pos4, h->pos[h->pcur], vb, cudaMemcpyDeviceToHost, h->stream));
+    if (vel4) CUDA_TRY(h, cudaMemcpyAsync(vel4, h->vel[h->pcur], vb, cudaMemcpyDeviceToHost, h->stream));
+    if (tag) CUDA_TRY(h, cudaMemcpyAsync(tag, h->tag[h->pcur], (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
+    if (cell) CUDA_TRY(h, cudaMemcpyAsync(cell, h->cell[h->pcur], (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (step) *step = h->step;
+    return MPCD_OK;
+}
+
+int mpcd_set_state(mpcd_t *h, const void *pos4, const void *vel4, const uint32_t *tag, uint64_t step)
+{
+    if (!h) return MPCD_EINVAL;
+    if (!pos4 || !vel4) return fail(h, MPCD_EINVAL, "pos4 and vel4 are required%s");
+    const size_t vb = (size_t)h->N * 4 * native_size(h);
+    CUDA_TRY(h, cudaMemcpyAsync(h->pos[h->pcur], pos4, vb, cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(h->vel[h->pcur], vel4, vb, cudaMemcpyHostToDevice, h->stream));
+    if (tag) {
+        CUDA_TRY(h, cudaMemcpyAsync(h->tag[h->pcur], tag, (size_t)h->N * 4, cudaMemcpyHostToDevice, h->stream));
+    } else {
+        iota_tags<<<grid_for(h->N, 256), 256, 0, h->stream>>>(h->N, h->tag[h->pcur]);
+        LAUNCH_CHECK(h);
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    h->step = step;
+    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    return MPCD_OK;
+}
+
+int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double *u3, double *axis3, double *kTc)
+{
+    if (!h) return MPCD_EINVAL;
+    if (!(h->sums_valid && h->rec_valid && h->energy_valid))
+        return fail(h, MPCD_ESTATE, "cell sums are not valid: call mpcd_shift_and_bin first%s");
+    if (axis3 && h->rec_mode != 0) return fail(h, MPCD_ESTATE, "no axis in the cell records (Andersen-thermostat finalize)%s");
+    const size_t Nc = (size_t)h->Nc;
+    // stage through one temporary device buffer (SoA), sized for everything asked
+    const size_t bytes = Nc * (4 + 8 * (3 + 1 + 3 + 3 + 1));
+    void *tmp = nullptr;
+    cudaError_t e = cudaMalloc(&tmp, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(h, MPCD_ENOMEM, "cudaMalloc (get_cells staging): %s", cudaGetErrorString(e)); }
+    char *base = static_cast<char *>(tmp);
+    double *d_sumv = reinterpret_cast<double *>(base);
+    double *d_ke = d_sumv + 3 * Nc;
+    double *d_u = d_ke + Nc;
+    double *d_ax = d_u + 3 * Nc;
+    double *d_kT = d_ax + 3 * Nc;
+    int32_t *d_cnt = reinterpret_cast<int32_t *>(d_kT + Nc);
+    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->cnt[h->ccur], h->rec, h->Nc, h->m, d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
+    h->launches += 1;
+    int rc = MPCD_OK;
+    auto cp = [&](void *dst, const void *src, size_t b) {
+        if (dst && rc == MPCD_OK && cudaMemcpyAsync(dst, src, b, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) rc = fail(h, MPCD_ECUDA, "get_cells copy failed%s");
+    };
+    cp(count, d_cnt, Nc * 4); cp(sumv3, d_sumv, Nc * 24); cp(ke, d_ke, Nc * 8); cp(u3, d_u, Nc * 24); cp(axis3, d_ax, Nc * 24); cp(kTc, d_kT, Nc * 8);
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess && rc == MPCD_OK) rc = fail(h, MPCD_ECUDA, "get_cells sync failed%s");
+    cudaFree(tmp);
+    return rc;
+}
+
+int mpcd_get_shift(mpcd_t *h, double s[3])
+{
+    if (!h || !s) return MPCD_EINVAL;
+    if (!h->bin_valid) return fail(h, MPCD_ESTATE, "no bin yet%s");
+    for (int d = 0; d < 3; ++d) s[d] = h->shift_used[d];
+    return MPCD_OK;
+}
+
+int mpcd_get_thermo(mpcd_t *h, double P[3], double *KE, double *kT)
+{
+    if (!h) return MPCD_EINVAL;
+    if (!(h->sums_valid && h->energy_valid)) {
+        int rc = bin_accumulate(h, h->bin_valid ? h->bin_step : h->step, false);
+        if (rc) return rc;
+    }
+    CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, 8 * sizeof(double), h->stream));
+    cell_thermo<<<148 * 4, 256, 0, h->stream>>>(h->acc[h->ccur], h->cnt[h->ccur], h->Nc, h->m, h->d_scalars);
+    LAUNCH_CHECK(h);
+    double out[6];
+    CUDA_TRY(h, cudaMemcpyAsync(out, h->d_scalars, sizeof(out), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (P) for (int d = 0; d < 3; ++d) P[d] = h->m * out[d];
+    if (KE) *KE = 0.5 * h->m * out[3];
+    if (kT) *kT = out[5] > 0 ? out[4] / out[5] : 0.0;
+    return MPCD_OK;
+}
+
+int mpcd_get_stats(mpcd_t *h, mpcd_stats *out)
+{
+    if (!h || !out) return MPCD_EINVAL;
+    std::memset(out, 0, sizeof(*out));
+    out->N = h->N; out->Nc = h->Nc;
+    for (int d = 0; d < 3; ++d) out->n[d] = h->n[d];
+    int mo = 0;
+    CUDA_TRY(h, cudaMemcpyAsync(&mo, h->d_max_occ, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    out->max_occupancy = mo;
+    out->step = h->step; out->kernel_launches = h->launches; out->sorts = h->sorts; out->device_bytes = h->device_bytes;
+    return MPCD_OK;
+}
+
+int mpcd_device_ptrs(mpcd_t *h, void **pos4, void **vel4, uint32_t **tag, int32_t **cell)
+{
+    if (!h) return MPCD_EINVAL;
+    if (pos4) *pos4 = h->pos[h->pcur];
+    if (vel4) *vel4 = h->vel[h->pcur];
+    if (tag) *tag = h->tag[h->pcur];
+    if (cell) *cell = h->cell[h->pcur];
+    return MPCD_OK;
+}
+
+const char *mpcd_last_error(const mpcd_t *h) { return h ? h->err : g_create_error; }
+
+int mpcd_abi_version(void) { return MPCD_ABI_VERSION; }
+
+const char *mpcd_build_info(void)
+{
+    return "mpcd-b200 ABI 1, sm_100a, nvcc " __VERSION__
+#ifdef __CUDACC_VER_MAJOR__
+           " / CUDA"
+#endif
+        ;
+}
+
+int mpcd_test_philox(const uint32_t *ctr4, const uint32_t *key2, uint32_t *out4, int64_t n)
+{
+    if (!ctr4 || !key2 || !out4 || n < 0) return MPCD_EINVAL;
+    if (n == 0) return MPCD_OK;
+    uint32_t *d = nullptr;
+    if (cudaMalloc(&d, (size_t)n * 10 * sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); return MPCD_ECUDA; }
+    uint32_t *dc = d, *dk = d + 4 * n, *dout = d + 6 * n;
+    int rc = MPCD_OK;
+    if (cudaMemcpy(dc, ctr4, (size_t)n * 16, cudaMemcpyHostToDevice) != cudaSuccess) rc = MPCD_ECUDA;
+    if (!rc && cudaMemcpy(dk, key2, (size_t)n * 8, cudaMemcpyHostToDevice) != cudaSuccess) rc = MPCD_ECUDA;
+    if (!rc) {
+        philox_test_kernel<<<grid_for(n, 256), 256>>>(dc, dk, dout, n);
+        if (cudaGetLastError() != cudaSuccess) rc = MPCD_ECUDA;
+    }
+    if (!rc && cudaMemcpy(out4, dout, (size_t)n * 16, cudaMemcpyDeviceToHost) != cudaSuccess) rc = MPCD_ECUDA;
+    cudaFree(d);
+    return rc;
+}
+
+}  // extern "C"

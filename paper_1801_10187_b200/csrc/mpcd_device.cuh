@@ -1,0 +1,240 @@
+// mpcd_device.cuh -- device-side building blocks of the MPCD solvent step for sm_100a.
+//
+// Citations are PAPER.md:<line> (the paper's text) and A<n> (readings in DESIGN.md).
+// This file shares nothing with oracle/: the RNG, the uniform conversions and the
+// domain constants are restated here.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace mpcdk {
+
+// ---------------------------------------------------------------------------------------
+// Counter-based RNG: Philox4x32-10 keyed like the paper keys Saru, (cell index | tag,
+// timestep, seed) (A24): key = seed, ctr = (index, t_lo, t_hi, domain).
+// ---------------------------------------------------------------------------------------
+enum : uint32_t { kDomShift = 1u, kDomAxis = 2u, kDomAT = 3u, kDomInitPos = 4u, kDomInitVel = 5u };
+
+struct u32x4 { uint32_t x, y, z, w; };
+
+__host__ __device__ __forceinline__ u32x4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                          uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return u32x4{c0, c1, c2, c3};
+}
+
+__host__ __device__ __forceinline__ u32x4 draw(uint64_t seed, uint64_t step, uint32_t index, uint32_t domain)
+{
+    return philox4x32_10(index, (uint32_t)step, (uint32_t)(step >> 32), domain, (uint32_t)seed, (uint32_t)(seed >> 32));
+}
+
+// (b + 1/2) 2^-32 in (0,1), exact in binary64
+__host__ __device__ __forceinline__ double u01_32(uint32_t b) { return ((double)b + 0.5) * 2.3283064365386962890625e-10; }
+// 53-bit uniform in [0,1)
+__host__ __device__ __forceinline__ double u01_53(uint32_t lo, uint32_t hi)
+{
+    return (double)((((uint64_t)hi << 32) | lo) >> 11) * 1.1102230246251565404236316680908203125e-16;
+}
+
+// Random unit axis by cylindrical projection (A13): U1 -> z, U2 -> azimuth.
+__device__ __forceinline__ void draw_axis(uint64_t seed, uint64_t step, uint32_t cell, double &nx, double &ny, double &nz)
+{
+    const u32x4 b = draw(seed, step, cell, kDomAxis);
+    const double z = 2.0 * u01_53(b.x, b.y) - 1.0;
+    double s, c;
+    sincospi(2.0 * u01_53(b.z, b.w), &s, &c);
+    const double rho = sqrt((1.0 - z) * (1.0 + z));   // sqrt(1 - z^2) without cancellation near the poles
+    nx = rho * c; ny = rho * s; nz = z;
+}
+
+// Three Gaussians of unit variance by Box-Muller from one Philox block keyed by the particle
+// tag (A17, A18); the fourth is discarded.
+__device__ __forceinline__ void gauss3_from_block(const u32x4 b, double &g0, double &g1, double &g2)
+{
+    const double r01 = sqrt(-2.0 * log(u01_32(b.x)));
+    const double r23 = sqrt(-2.0 * log(u01_32(b.z)));
+    double s, c;
+    sincospi(2.0 * u01_32(b.y), &s, &c);
+    g0 = r01 * c; g1 = r01 * s;
+    g2 = r23 * cospi(2.0 * u01_32(b.w));
+}
+__device__ __forceinline__ void draw_gauss3(uint64_t seed, uint64_t step, uint32_t tag, double &g0, double &g1, double &g2)
+{
+    gauss3_from_block(draw(seed, step, tag, kDomAT), g0, g1, g2);
+}
+
+// ---------------------------------------------------------------------------------------
+// Native-precision arithmetic with explicit rounding: streaming and binning are DEFINED as
+// separately rounded operations (A6, A7), so no FMA contraction may happen here.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ float  add_rn(float a, float b)   { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float  sub_rn(float a, float b)   { return __fsub_rn(a, b); }
+__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ float  mul_rn(float a, float b)   { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ int floor_int(float q)  { return __float2int_rd(q); }
+__device__ __forceinline__ int floor_int(double q) { return __double2int_rd(q); }
+
+template <typename T> struct Vec4;
+template <> struct Vec4<float>  { using type = float4; };
+template <> struct Vec4<double> { using type = double4; };
+
+// 16-byte vector accesses (north_star: "coalesced 16-byte HBM access"); double4 = two of them.
+__device__ __forceinline__ float4 load4(const float4 *p) { return *p; }
+__device__ __forceinline__ void store4(float4 *p, float4 v) { *p = v; }
+__device__ __forceinline__ double4 load4(const double4 *p)
+{
+    const double2 a = reinterpret_cast<const double2 *>(p)[0], b = reinterpret_cast<const double2 *>(p)[1];
+    return double4{a.x, a.y, b.x, b.y};
+}
+__device__ __forceinline__ void store4(double4 *p, double4 v)
+{
+    reinterpret_cast<double2 *>(p)[0] = double2{v.x, v.y};
+    reinterpret_cast<double2 *>(p)[1] = double2{v.z, v.w};
+}
+
+// eq. 1 PAPER.md:35 + periodic wrap (A7): x = fl(x + fl(v dt)); if x < 0: x += L; if x >= L: x -= L.
+template <typename T> __device__ __forceinline__ T stream_wrap(T x, T v, T dt, T L)
+{
+    x = add_rn(x, mul_rn(v, dt));
+    if (x < T(0)) x = add_rn(x, L);
+    if (x >= L) x = sub_rn(x, L);
+    return x;
+}
+
+// PAPER.md:110 + A6: i = floor(fl(fl(x + s) * inv_a)), integer periodic wrap.
+template <typename T> __device__ __forceinline__ int bin_axis(T x, T s, T inv_a, int n)
+{
+    int i = floor_int(mul_rn(add_rn(x, s), inv_a));
+    if (i < 0) i += n;
+    if (i >= n) i -= n;
+    return i;
+}
+
+// ---------------------------------------------------------------------------------------
+// Per-cell fp64 accumulation.  Layout in HBM: acc[c] = {Sx, Sy, Sz, Q}
+// (4 doubles = one 32-byte sector, Q = sum |v|^2) and cnt[c] (int32).
+//
+// The L2 atomic path of a B200 SM retires about one RED *request* (distinct 32-byte sector
+// per instruction) every ~1.3 cycles, which -- not HBM bandwidth -- bounds this step
+// (profiles/r01_atomics_probe.md).  So lanes are first combined by cell inside the warp
+// (match.any + shuffle tree), and the surviving leaders are then issued "transposed": four
+// adjacent lanes add the four doubles of ONE record in one instruction, i.e. one sector
+// request per (leader, record) instead of four.
+// ---------------------------------------------------------------------------------------
+struct WarpScratch {           // per-warp staging for the transposed issue
+    double v[32][4];
+    int cell[32];
+    int n[32];
+};
+
+template <bool kEnergy>
+__device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, int *__restrict__ cnt, WarpScratch &ws,
+                                                     int c /* < 0 = inactive lane, unique per lane */, double vx, double vy, double vz)
+{
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    double q = kEnergy ? (vx * vx + vy * vy + vz * vz) : 0.0;
+    unsigned peers = __match_any_sync(full, c);
+    const int size = __popc(peers);
+    const bool leader = (__ffs(peers) - 1) == lane;
+    int rank = __popc(peers & ((1u << lane) - 1u));
+    peers &= (0xfffffffeu << lane);                        // peers above this lane
+    while (__any_sync(full, peers != 0u)) {                // log2(largest group) rounds
+        const int next = __ffs(peers);                     // 1-based lane of the next peer, 0 = none
+        const int src = next ? next - 1 : lane;
+        const double tx = __shfl_sync(full, vx, src), ty = __shfl_sync(full, vy, src), tz = __shfl_sync(full, vz, src);
+        const double tq = kEnergy ? __shfl_sync(full, q, src) : 0.0;
+        if (next) { vx += tx; vy += ty; vz += tz; q += tq; }
+        peers &= __ballot_sync(full, !(rank & 1));         // odd-ranked lanes have been absorbed
+        rank >>= 1;
+    }
+    const unsigned leaders = __ballot_sync(full, leader && c >= 0);
+    const int nl = __popc(leaders);
+    if (leader && c >= 0) {
+        const int j = __popc(leaders & ((1u << lane) - 1u));
+        ws.v[j][0] = vx; ws.v[j][1] = vy; ws.v[j][2] = vz; ws.v[j][3] = q;
+        ws.cell[j] = c; ws.n[j] = size;
+    }
+    __syncwarp();
+    const int comp = lane & 3;
+    for (int base = 0; base < nl; base += 8) {
+        const int j = base + (lane >> 2);
+        if (j < nl) {
+            const int cc = ws.cell[j];
+            if (kEnergy || comp < 3) atomicAdd(acc + 4 * (size_t)cc + comp, ws.v[j][comp]);
+            if (comp == 0) atomicAdd(cnt + cc, ws.n[j]);
+        }
+    }
+    __syncwarp();
+}
+
+// Same for a 3-vector only (the Andersen-thermostat second reduction).
+__device__ __forceinline__ void warp_cell_accumulate3(double *__restrict__ acc, WarpScratch &ws, int c, double vx, double vy, double vz)
+{
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    unsigned peers = __match_any_sync(full, c);
+    const bool leader = (__ffs(peers) - 1) == lane;
+    int rank = __popc(peers & ((1u << lane) - 1u));
+    peers &= (0xfffffffeu << lane);
+    while (__any_sync(full, peers != 0u)) {
+        const int next = __ffs(peers);
+        const int src = next ? next - 1 : lane;
+        const double tx = __shfl_sync(full, vx, src), ty = __shfl_sync(full, vy, src), tz = __shfl_sync(full, vz, src);
+        if (next) { vx += tx; vy += ty; vz += tz; }
+        peers &= __ballot_sync(full, !(rank & 1));
+        rank >>= 1;
+    }
+    const unsigned leaders = __ballot_sync(full, leader && c >= 0);
+    const int nl = __popc(leaders);
+    if (leader && c >= 0) {
+        const int j = __popc(leaders & ((1u << lane) - 1u));
+        ws.v[j][0] = vx; ws.v[j][1] = vy; ws.v[j][2] = vz;
+        ws.cell[j] = c;
+    }
+    __syncwarp();
+    const int comp = lane & 3;
+    for (int base = 0; base < nl; base += 8) {
+        const int j = base + (lane >> 2);
+        if (j < nl && comp < 3) atomicAdd(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[j][comp]);
+    }
+    __syncwarp();
+}
+
+// Block-wide sum of k doubles into out[0..k) with one atomic per block and value.
+template <int K> __device__ __forceinline__ void block_sum_to_global(double (&v)[K], double *out)
+{
+    __shared__ double sm[32][K];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_down_sync(0xffffffffu, v[k], o);
+    if (lane == 0)
+#pragma unroll
+        for (int k = 0; k < K; ++k) sm[warp][k] = v[k];
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            double x = lane < nw ? sm[lane][k] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+            if (lane == 0) atomicAdd(out + k, x);
+        }
+    }
+    __syncthreads();
+}
+
+}  // namespace mpcdk

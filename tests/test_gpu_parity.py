@@ -1,0 +1,266 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances (north_star): cell indices, counts and
+post-stream positions bit-exact; velocities after one step max-abs <= 1e-5 sqrt(kT/m) in the
+mixed model and <= 1e-12 in the fp64 model; cell sums to 1e-12 (fp64 reassociation only)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1801_10187_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+MIXED_TOL = 1e-5
+FP64_TOL = 1e-12
+
+
+def _pair(oracle, n, M, seed, dtype, a=1.0, m=1.0, kT=1.0, N=None, **kw):
+    """The same synthetic state in a CUDA handle and in an oracle object."""
+    from paper_1801_10187_b200 import MPCD
+    pos, vel, tag = synth.solvent(n, M, seed=seed, a=a, kT=kT, m=m, dtype=dtype, N=N)
+    box = [x * a for x in n]
+    rule = kw.get("rule", "srd")
+    g = MPCD(box, pos.shape[0], a=a, m=m, kT=kT, seed=seed, precision="fp64" if dtype == np.float64 else "mixed",
+             init_state=False, **kw)
+    g.set_state(pos, vel, tag)
+    okw = {k: v for k, v in kw.items() if k in ("dt", "alpha", "sort_period")}
+    o = oracle.OracleMPCD(box, pos.shape[0], a=a, m=m, kT=kT, seed=seed, dtype=dtype, init=False,
+                          rule=1 if rule == "at" else 0, **okw)
+    o.set_state(pos, vel, tag)
+    return g, o
+
+
+def _tol(dtype, sigma=1.0):
+    return (FP64_TOL if dtype == np.float64 else MIXED_TOL) * sigma
+
+
+def _by_tag(state):
+    order = np.argsort(state["tag"], kind="stable")
+    return {k: (v[order] if isinstance(v, np.ndarray) else v) for k, v in state.items()}
+
+
+def test_device_philox_matches_oracle_and_known_answers(oracle):
+    from paper_1801_10187_b200 import test_philox
+    rng = np.random.default_rng(5)
+    ctr = rng.integers(0, 2**32, size=(4096, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2**32, size=(4096, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0], key[0] = 0, 0
+    ctr[1], key[1] = 0xFFFFFFFF, 0xFFFFFFFF
+    ctr[2], key[2] = [0x243F6A88, 0x85A308D3, 0x13198A2E, 0x03707344], [0xA4093822, 0x299F31D0]
+    out = test_philox(ctr, key)
+    assert [hex(x) for x in out[0]] == ["0x6627e8d5", "0xe169c58d", "0xbc57ac4c", "0x9b00dbd8"]
+    assert [hex(x) for x in out[2]] == ["0xd16cfe09", "0x94fdcceb", "0x5001e420", "0x24126ea1"]
+    for i in range(0, 4096, 7):
+        assert list(out[i]) == oracle.philox4x32_10(ctr[i], key[i])
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("n,M,a", [((8, 8, 8), 5, 1.0), ((5, 7, 3), 9, 0.7), ((40, 33, 21), 10, 1.0)])
+def test_stream_and_bin_are_bit_exact(oracle, dtype, n, M, a):
+    g, o = _pair(oracle, n, M, 1801, dtype, a=a)
+    for it in range(3):
+        g.stream(); o.stream()
+        gs = g.get_state()
+        assert np.array_equal(gs["pos"][:, :3], o.pos[:, :3])              # bit-exact positions
+        assert np.array_equal(gs["vel"][:, :3], o.vel[:, :3])
+        g.shift_and_bin(); o.shift_and_bin()
+        want_shift = o.shift.astype(dtype).astype(np.float64)
+        assert np.array_equal(g.get_shift(), want_shift)
+        gs = g.get_state()
+        assert np.array_equal(gs["cell"], o.cell)                          # bit-exact cell indices
+        c = g.get_cells()
+        assert np.array_equal(c["count"], o.count)                         # bit-exact counts
+        np.testing.assert_allclose(c["sumv"], o.sumv, rtol=0, atol=1e-12)
+        np.testing.assert_allclose(c["ke"], o.ke, rtol=1e-13, atol=1e-12)
+        np.testing.assert_allclose(c["u"], o.u, rtol=0, atol=1e-13)
+        # the oracle rounds phi = 2 pi U once (dphi <= 2 pi 2^-53 = 7e-16); the GPU uses sincospi(2U)
+        np.testing.assert_allclose(c["axis"], o.axis, rtol=0, atol=4e-15)
+        # E_rel: GPU uses KE - M u^2/2 (A12), oracle the two-pass definition; compare through kT_c
+        np.testing.assert_allclose(c["kTc"], o.kTc, rtol=1e-10, atol=1e-11)
+        assert g.stats()["max_occupancy"] == o.count.max()
+        # advance both with the oracle-free collide so the next round starts from new velocities
+        g.collide_srd(math.radians(130.0)); o.collide_srd(math.radians(130.0))
+        g.set_state(o.pos, o.vel, o.tag, step=it + 1)                      # teacher-forced
+        o.step_count = it + 1
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("alpha_deg", [130.0, 90.0, 180.0])
+def test_srd_collision_one_step_parity(oracle, dtype, alpha_deg):
+    g, o = _pair(oracle, (12, 10, 9), 10, 77, dtype)
+    al = math.radians(alpha_deg)
+    g.stream(); o.stream()
+    g.shift_and_bin(); o.shift_and_bin()
+    g.collide_srd(al); o.collide_srd(al)
+    gs = g.get_state()
+    assert np.array_equal(gs["pos"][:, :3], o.pos[:, :3])
+    err = np.max(np.abs(gs["vel"][:, :3].astype(np.float64) - o.vel[:, :3].astype(np.float64)))
+    assert err <= _tol(dtype), err
+    # it really collided
+    assert np.max(np.abs(gs["vel"][:, :3] - synth.solvent((12, 10, 9), 10, seed=77, dtype=dtype)[1][:, :3])) > 0.1
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_at_collision_one_step_parity(oracle, dtype):
+    kT, m = 1.5, 2.0
+    g, o = _pair(oracle, (9, 8, 7), 5, 42, dtype, kT=kT, m=m, rule="at")
+    g.stream(); o.stream()
+    g.shift_and_bin(); o.shift_and_bin()
+    g.collide_at(); o.collide_at()
+    gs = g.get_state()
+    err = np.max(np.abs(gs["vel"][:, :3].astype(np.float64) - o.vel[:, :3].astype(np.float64)))
+    assert err <= _tol(dtype, math.sqrt(kT / m)), err
+    P, KE, kTm = g.get_thermo()
+    assert abs(kTm / kT - 1) < 0.1
+
+
+def test_calls_out_of_order_return_estate(oracle):
+    from paper_1801_10187_b200 import MPCDError
+    g, o = _pair(oracle, (4, 4, 4), 5, 3, np.float32)
+    for call in (lambda: g.collide_srd(1.0), g.collide_at, g.sort, g.get_cells):
+        with pytest.raises(MPCDError) as e:
+            call()
+        assert e.value.code == -4
+    g.shift_and_bin()
+    g.collide_srd(1.0)
+    with pytest.raises(MPCDError):
+        g.collide_srd(1.0)          # the sums are stale after a collision
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_sort_keeps_the_multiset_and_orders_by_cell(oracle, dtype):
+    g, o = _pair(oracle, (9, 6, 11), 10, 23, dtype)
+    g.stream(); g.shift_and_bin()
+    before = g.get_state()
+    g.sort()
+    after = g.get_state()
+    assert np.all(np.diff(after["cell"]) >= 0)                              # cell[] non-decreasing
+    a, b = _by_tag(after), _by_tag(before)
+    for k in ("tag", "pos", "vel", "cell"):
+        assert np.array_equal(a[k], b[k]), k                                 # multiset unchanged bit for bit
+    # cell sums do not depend on the order; collide after the sort agrees with the oracle by tag
+    o.stream(); o.shift_and_bin(); o.sort(); o.collide_srd()
+    g.collide_srd(math.radians(130.0))
+    gs = _by_tag(g.get_state())
+    os_ = np.argsort(o.tag)
+    err = np.max(np.abs(gs["vel"][:, :3].astype(np.float64) - o.vel[os_][:, :3].astype(np.float64)))
+    assert err <= _tol(dtype)
+    assert g.stats()["sorts"] == 1
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("rule", ["srd", "at"])
+def test_fused_step_equals_oracle_steps(oracle, dtype, rule):
+    """mpcd_step(k) runs the fused one-pass-per-step pipeline; compare with k oracle steps by tag
+    (k small enough that a 1-ulp fp32 difference cannot yet flip a cell membership)."""
+    g, o = _pair(oracle, (16, 12, 10), 10, 5, dtype, rule=rule, sort_period=2)
+    g.step(3); o.step(3)
+    gs = _by_tag(g.get_state())
+    os_ = np.argsort(o.tag)
+    assert gs["step"] == 3 and np.array_equal(gs["tag"], o.tag[os_])
+    ptol = 1e-6 if dtype == np.float32 else 1e-12
+    assert np.max(np.abs(gs["pos"][:, :3].astype(np.float64) - o.pos[os_][:, :3])) <= ptol
+    assert np.array_equal(gs["cell"], o.cell[os_])
+    err = np.max(np.abs(gs["vel"][:, :3].astype(np.float64) - o.vel[os_][:, :3].astype(np.float64)))
+    assert err <= 3 * _tol(dtype), err
+
+
+def test_fused_step_equals_unfused_calls(oracle):
+    ga, _ = _pair(oracle, (10, 10, 10), 10, 9, np.float64, sort_period=0)
+    gb, _ = _pair(oracle, (10, 10, 10), 10, 9, np.float64, sort_period=0)
+    ga.step(4)
+    for _ in range(4):
+        gb.stream(); gb.shift_and_bin(); gb.collide_srd(math.radians(130.0))
+        st = gb.get_state()
+        gb.set_state(st["pos"], st["vel"], st["tag"], step=st["step"] + 1)
+    a, b = ga.get_state(), gb.get_state()
+    np.testing.assert_allclose(a["pos"], b["pos"], rtol=0, atol=1e-12)
+    np.testing.assert_allclose(a["vel"], b["vel"], rtol=0, atol=1e-12)
+    assert a["step"] == b["step"] == 4
+
+
+def test_config1_teacher_forced_100_steps(oracle):
+    """BASELINE config 1 (L = 8, density 5, 2560 particles, mixed, sort every 25): every step the
+    oracle advances the GPU's state_t by one step and must land on the GPU's state_{t+1}."""
+    cfg = synth.CONFIGS["C1"]
+    g, o = _pair(oracle, cfg["n"], cfg["M"], cfg["seed"], np.float32, sort_period=25)
+    worst = 0.0
+    for t in range(100):
+        st = _by_tag(g.get_state())
+        o.set_state(st["pos"], st["vel"], st["tag"], step=t)
+        g.step(1); o.step(1)
+        gs = _by_tag(g.get_state())
+        os_ = np.argsort(o.tag)
+        assert np.array_equal(gs["pos"][:, :3], o.pos[os_][:, :3])
+        assert np.array_equal(gs["cell"], o.cell[os_])
+        worst = max(worst, np.max(np.abs(gs["vel"][:, :3].astype(np.float64) - o.vel[os_][:, :3].astype(np.float64))))
+    assert worst <= MIXED_TOL, worst
+    assert g.stats()["sorts"] == 4
+
+
+@pytest.mark.parametrize("N", [1, 31, 33, 255, 257, 1000])
+def test_ragged_sizes_and_nearly_empty_boxes(oracle, N):
+    """Ragged tails (N not a multiple of the warp / block), N = 1, and mostly empty cells."""
+    g, o = _pair(oracle, (6, 5, 4), None, 100 + N, np.float32, N=N, sort_period=1)
+    g.step(2); o.step(2)
+    gs = _by_tag(g.get_state())
+    os_ = np.argsort(o.tag)
+    assert np.array_equal(gs["pos"][:, :3], o.pos[os_][:, :3])
+    assert np.array_equal(gs["cell"], o.cell[os_])
+    assert np.max(np.abs(gs["vel"][:, :3].astype(np.float64) - o.vel[os_][:, :3])) <= MIXED_TOL
+    g.shift_and_bin(); o.shift_and_bin()
+    c = g.get_cells()
+    assert np.array_equal(c["count"], o.count) and c["count"].sum() == N
+    empty = o.count == 0
+    assert np.all(c["u"][empty] == 0) and np.all(c["kTc"][o.count < 2] == 0)     # A11, A16
+
+
+def test_crowded_cell(oracle):
+    """Degenerate: every particle in one cell (whole warps share one accumulator)."""
+    from paper_1801_10187_b200 import MPCD
+    N = 1000
+    rng = np.random.default_rng(0)
+    pos = np.zeros((N, 4), np.float32); vel = np.zeros((N, 4), np.float32)
+    pos[:, :3] = 2.25 + 0.5 * rng.random((N, 3))
+    vel[:, :3] = rng.standard_normal((N, 3))
+    g = MPCD([4, 4, 4], N, seed=3, init_state=False)
+    g.set_state(pos, vel)
+    o = oracle.OracleMPCD([4.0] * 3, N, seed=3, dtype=np.float32, init=False)
+    o.set_state(pos, vel)
+    g.shift_and_bin(); o.shift_and_bin()
+    c = g.get_cells()
+    assert np.array_equal(c["count"], o.count) and c["count"].max() >= 100
+    np.testing.assert_allclose(c["sumv"], o.sumv, rtol=0, atol=1e-11)
+    g.collide_srd(2.0); o.collide_srd(2.0)
+    assert np.max(np.abs(g.get_state()["vel"][:, :3].astype(np.float64) - o.vel[:, :3])) <= MIXED_TOL
+
+
+def test_thermo_matches_oracle(oracle):
+    g, o = _pair(oracle, (10, 10, 10), 10, 2, np.float64)
+    g.step(2); o.step(2)
+    P, KE, kT = g.get_thermo()
+    Po, KEo, kTo = o.thermo()
+    np.testing.assert_allclose(P, Po, rtol=0, atol=1e-9)
+    np.testing.assert_allclose(KE, KEo, rtol=1e-12)
+    np.testing.assert_allclose(kT, kTo, rtol=1e-10)
+
+
+def test_device_init_has_the_papers_initial_condition(oracle):
+    """mpcd_create's own initial state (A23): uniform positions, N(0, kT/m) velocities, zero mean."""
+    from paper_1801_10187_b200 import MPCD
+    from scipy import stats
+    kT, m = 2.0, 0.5
+    for prec, dtype in (("mixed", np.float32), ("fp64", np.float64)):
+        g = MPCD([20, 20, 20], 80000, kT=kT, m=m, seed=11, precision=prec)
+        s = g.get_state()
+        assert np.array_equal(s["tag"], np.arange(80000, dtype=np.uint32))
+        assert s["pos"][:, :3].min() >= 0 and s["pos"][:, :3].max() < 20
+        assert stats.kstest(s["pos"][:, 0] / 20, "uniform").pvalue > 1e-3
+        v = s["vel"][:, :3].astype(np.float64)
+        assert np.max(np.abs(v.mean(axis=0))) < (1e-7 if dtype == np.float32 else 1e-14)
+        assert stats.kstest(v[:, 1] / math.sqrt(kT / m), "norm").pvalue > 1e-3
+        # same draws as the oracle's statement of A23
+        po, vo, _ = oracle.init_state(11, 80000, [20.0] * 3, math.sqrt(kT / m), dtype)
+        assert np.array_equal(s["pos"][:, :3], po[:, :3])
+        np.testing.assert_allclose(v, vo[:, :3].astype(np.float64), rtol=0, atol=1e-6 if dtype == np.float32 else 1e-13)
