@@ -177,6 +177,20 @@ typedef struct mpcd_stats {
 } mpcd_stats;
 int mpcd_get_stats(mpcd_t *h, mpcd_stats *out /* host */);
 
+/* Opt-in per-kernel timing.  While on, every launch group is bracketed by a CUDA event
+ * pair on the handle's stream (this costs a little, so leave it off for throughput runs).
+ * mpcd_get_profile synchronises and returns, per kind, the summed device time in ms and the
+ * number of launch groups since profiling was switched on.  ms, count: host, may be NULL. */
+#define MPCD_PROF_FUSED    0   /* collide(t) + stream + bin + accumulate(t+1): the steady-state step kernel */
+#define MPCD_PROF_BIN      1   /* [stream +] bin + accumulate without a collision */
+#define MPCD_PROF_COLLIDE  2   /* collision only */
+#define MPCD_PROF_FINALIZE 3   /* per-cell finalize (u, kT_c, axis) */
+#define MPCD_PROF_SORT     4   /* scan + scatter */
+#define MPCD_PROF_OTHER    5
+#define MPCD_PROF_KINDS    6
+int mpcd_set_profiling(mpcd_t *h, int32_t on);
+int mpcd_get_profile(mpcd_t *h, double ms[MPCD_PROF_KINDS], uint64_t count[MPCD_PROF_KINDS]);
+
 /* DEVICE pointers of the current particle arrays (for zero-copy inspection; they
  * change after a sort).  Any output may be NULL. */
 int mpcd_device_ptrs(mpcd_t *h, void **pos4, void **vel4, uint32_t **tag, int32_t **cell);

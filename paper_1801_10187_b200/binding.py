@@ -50,8 +50,9 @@ EXPORTS = [
     "mpcd_default_options", "mpcd_create", "mpcd_create_ex", "mpcd_destroy", "mpcd_stream", "mpcd_shift_and_bin",
     "mpcd_collide_srd", "mpcd_collide_at", "mpcd_sort", "mpcd_step", "mpcd_get_state", "mpcd_set_state",
     "mpcd_get_cells", "mpcd_get_shift", "mpcd_get_thermo", "mpcd_get_stats", "mpcd_device_ptrs", "mpcd_last_error",
-    "mpcd_abi_version", "mpcd_build_info", "mpcd_test_philox",
+    "mpcd_abi_version", "mpcd_build_info", "mpcd_test_philox", "mpcd_set_profiling", "mpcd_get_profile",
 ]
+PROF_KINDS = ("fused", "bin", "collide", "finalize", "sort", "other")
 
 _lib = None
 
@@ -85,6 +86,8 @@ def load_library():
     lib.mpcd_last_error.restype = C.c_char_p
     lib.mpcd_build_info.restype = C.c_char_p
     lib.mpcd_test_philox.argtypes = [vp, vp, vp, i64]
+    lib.mpcd_set_profiling.argtypes = [vp, i32]
+    lib.mpcd_get_profile.argtypes = [vp, P(dbl), P(u64)]
     for name in EXPORTS:
         if name not in ("mpcd_last_error", "mpcd_build_info"):
             getattr(lib, name).restype = C.c_int
@@ -245,6 +248,16 @@ class MPCD:
         self._check(self.lib.mpcd_get_stats(self.h, C.byref(s)))
         return dict(N=s.N, Nc=s.Nc, n=tuple(s.n), max_occupancy=s.max_occupancy, step=s.step,
                     kernel_launches=s.kernel_launches, sorts=s.sorts, device_bytes=s.device_bytes)
+
+    def set_profiling(self, on=True):
+        self._check(self.lib.mpcd_set_profiling(self.h, int(bool(on))))
+
+    def get_profile(self):
+        """{kind: (summed ms, launch groups)} since profiling was switched on."""
+        ms = (C.c_double * len(PROF_KINDS))()
+        n = (C.c_uint64 * len(PROF_KINDS))()
+        self._check(self.lib.mpcd_get_profile(self.h, ms, n))
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(PROF_KINDS)}
 
     def synchronize(self):
         self._stream.synchronize()

@@ -53,6 +53,12 @@ struct mpcd {
     // bookkeeping
     std::vector<Buffer> buffers;
     uint64_t launches = 0, sorts = 0, device_bytes = 0;
+    // opt-in per-kernel timing (mpcd_set_profiling): CUDA events on the handle's stream
+    bool profiling = false;
+    struct Timed { cudaEvent_t a, b; int kind; };
+    std::vector<Timed> timed;
+    double prof_ms[MPCD_PROF_KINDS] = {0};
+    uint64_t prof_n[MPCD_PROF_KINDS] = {0};
     char err[256] = "no error";
 };
 
@@ -100,6 +106,36 @@ template <typename P> int dev_alloc_t(mpcd_t *h, P **out, size_t count) { return
 
 inline size_t native_size(const mpcd_t *h) { return h->opt.precision == MPCD_FP64 ? sizeof(double) : sizeof(float); }
 inline unsigned grid_for(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+struct ProfScope {   // brackets the launches of one kind with a CUDA event pair when profiling is on
+    mpcd_t *h; int kind; cudaEvent_t a = nullptr, b = nullptr;
+    ProfScope(mpcd_t *h_, int kind_) : h(h_), kind(kind_)
+    {
+        if (!h->profiling) return;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { a = b = nullptr; return; }
+        cudaEventRecord(a, h->stream);
+    }
+    ~ProfScope()
+    {
+        if (!a) return;
+        cudaEventRecord(b, h->stream);
+        h->timed.push_back(mpcd::Timed{a, b, kind});
+    }
+};
+
+void drain_profile(mpcd_t *h)
+{
+    for (const auto &t : h->timed) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(t.b) == cudaSuccess && cudaEventElapsedTime(&ms, t.a, t.b) == cudaSuccess) {
+            h->prof_ms[t.kind] += ms;
+            h->prof_n[t.kind] += 1;
+        }
+        cudaEventDestroy(t.a);
+        cudaEventDestroy(t.b);
+    }
+    h->timed.clear();
+}
 
 // a2: the step's grid shift, uniform on (-a/2, a/2)^3 from Philox(seed, (0, t, SHIFT)) (A4, A5)
 void draw_shift(const mpcd_t *h, uint64_t step, double s[3])
@@ -170,6 +206,8 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, int acc_set, uint64
 
 int pass(mpcd_t *h, unsigned F, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
 {
+    const bool collide = (F & (kSRD | kATApply)) != 0, bin = (F & kBin) != 0;
+    ProfScope prof(h, collide && bin ? MPCD_PROF_FUSED : (collide ? MPCD_PROF_COLLIDE : (bin ? MPCD_PROF_BIN : MPCD_PROF_OTHER)));
     return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, acc_set, step_collide, step_bin, shift, alpha)
                                          : launch_pass<float>(h, F, acc_set, step_collide, step_bin, shift, alpha);
 }
@@ -212,6 +250,7 @@ int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool z
     f.max_occupancy = h->d_max_occ;
     f.Nc = h->Nc; f.m = h->m; f.seed = h->seed; f.step = t;
     f.at_mode = at_mode; f.have_energy = have_energy ? 1 : 0;
+    ProfScope prof(h, MPCD_PROF_FINALIZE);
     CUDA_TRY(h, cudaMemsetAsync(h->d_max_occ, 0, sizeof(int), h->stream));
     cell_finalize<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(f);
     LAUNCH_CHECK(h);
@@ -226,6 +265,7 @@ int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool z
 int do_sort(mpcd_t *h, int s)
 {
     const int ntiles = (int)((h->Nc + kScanTile - 1) / kScanTile);
+    ProfScope prof(h, MPCD_PROF_SORT);
     scan_tile_sums<<<ntiles, kScanThreads, 0, h->stream>>>(h->cnt[s], h->Nc, h->tile_sum);
     LAUNCH_CHECK(h);
     scan_tile_offsets<<<1, 1024, 0, h->stream>>>(h->tile_sum, ntiles);
@@ -398,6 +438,7 @@ int mpcd_destroy(mpcd_t *h)
 {
     if (!h) return MPCD_EINVAL;
     cudaStreamSynchronize(h->stream);
+    drain_profile(h);
     release(h);
     delete h;
     return MPCD_OK;
@@ -624,6 +665,28 @@ int mpcd_device_ptrs(mpcd_t *h, void **pos4, void **vel4, uint32_t **tag, int32_
     if (vel4) *vel4 = h->vel[h->pcur];
     if (tag) *tag = h->tag[h->pcur];
     if (cell) *cell = h->cell[h->pcur];
+    return MPCD_OK;
+}
+
+int mpcd_set_profiling(mpcd_t *h, int32_t on)
+{
+    if (!h) return MPCD_EINVAL;
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    drain_profile(h);
+    h->profiling = on != 0;
+    for (int k = 0; k < MPCD_PROF_KINDS; ++k) { h->prof_ms[k] = 0; h->prof_n[k] = 0; }
+    return MPCD_OK;
+}
+
+int mpcd_get_profile(mpcd_t *h, double ms[MPCD_PROF_KINDS], uint64_t count[MPCD_PROF_KINDS])
+{
+    if (!h) return MPCD_EINVAL;
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    drain_profile(h);
+    for (int k = 0; k < MPCD_PROF_KINDS; ++k) {
+        if (ms) ms[k] = h->prof_ms[k];
+        if (count) count[k] = h->prof_n[k];
+    }
     return MPCD_OK;
 }
 
