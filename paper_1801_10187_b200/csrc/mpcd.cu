@@ -7,6 +7,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -39,7 +40,7 @@ struct mpcd {
     double *acc[2] = {nullptr, nullptr};
     int32_t *cnt[2] = {nullptr, nullptr};
     double *at_acc[2] = {nullptr, nullptr};
-    CellRec *rec = nullptr;
+    CellRec *rec[2] = {nullptr, nullptr};   // per accumulator set (step parity)
     int32_t *cell_start = nullptr, *tile_sum = nullptr;
     int *d_max_occ = nullptr;
     double *d_scalars = nullptr;   // 8 doubles of scratch for reductions
@@ -145,14 +146,15 @@ void draw_shift(const mpcd_t *h, uint64_t step, double s[3])
     for (int d = 0; d < 3; ++d) s[d] = (u01_32(w[d]) - 0.5) * h->a;
 }
 
-template <typename T> PassArgs<T> make_args(mpcd_t *h, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
+template <typename T> PassArgs<T> make_args(mpcd_t *h, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3],
+                                            double alpha)
 {
     PassArgs<T> a{};
     a.pos = static_cast<typename Vec4<T>::type *>(h->pos[h->pcur]);
     a.vel = static_cast<typename Vec4<T>::type *>(h->vel[h->pcur]);
     a.tag = h->tag[h->pcur];
     a.cell = h->cell[h->pcur];
-    a.rec = h->rec;
+    a.rec = h->rec[rec_set];
     a.acc = h->acc[acc_set];
     a.cnt = h->cnt[acc_set];
     a.at_acc = h->at_acc[acc_set];
@@ -178,13 +180,13 @@ template <typename T, unsigned F> void launch_pass_t(mpcd_t *h, const PassArgs<T
     particle_pass<T, F><<<grid_for(h->N, kPassThreads), kPassThreads, 0, h->stream>>>(a);
 }
 
-template <typename T> int launch_pass(mpcd_t *h, unsigned F, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
+template <typename T> int launch_pass(mpcd_t *h, unsigned F, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin,
+                                      const double shift[3], double alpha)
 {
-    const PassArgs<T> a = make_args<T>(h, acc_set, step_collide, step_bin, shift, alpha);
+    const PassArgs<T> a = make_args<T>(h, rec_set, acc_set, step_collide, step_bin, shift, alpha);
     switch (F) {
 #define CASE(f) case (f): launch_pass_t<T, (f)>(h, a); break;
         CASE(kStream)
-        CASE(kBin)
         CASE(kBin | kEnergy)
         CASE(kStream | kBin)
         CASE(kStream | kBin | kEnergy)
@@ -204,12 +206,12 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, int acc_set, uint64
     return MPCD_OK;
 }
 
-int pass(mpcd_t *h, unsigned F, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
+int pass(mpcd_t *h, unsigned F, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
 {
     const bool collide = (F & (kSRD | kATApply)) != 0, bin = (F & kBin) != 0;
     ProfScope prof(h, collide && bin ? MPCD_PROF_FUSED : (collide ? MPCD_PROF_COLLIDE : (bin ? MPCD_PROF_BIN : MPCD_PROF_OTHER)));
-    return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, acc_set, step_collide, step_bin, shift, alpha)
-                                         : launch_pass<float>(h, F, acc_set, step_collide, step_bin, shift, alpha);
+    return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, rec_set, acc_set, step_collide, step_bin, shift, alpha)
+                                         : launch_pass<float>(h, F, rec_set, acc_set, step_collide, step_bin, shift, alpha);
 }
 
 int ensure_at_buffers(mpcd_t *h)
@@ -235,7 +237,7 @@ int zero_set(mpcd_t *h, int s, bool sums, bool at)
     return MPCD_OK;
 }
 
-// a5 for accumulator set `s` at step `t`; optionally zero the other set for the next step.
+// a5 for accumulator set `s` at step `t` into rec[s]; optionally zero the other set for the next step.
 int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool zero_next)
 {
     FinalizeArgs f{};
@@ -246,13 +248,13 @@ int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool z
     f.acc_next = zs ? h->acc[o] : nullptr;
     f.cnt_next = zs ? h->cnt[o] : nullptr;
     f.at_acc_next = za ? h->at_acc[o] : nullptr;
-    f.rec = h->rec;
+    f.rec = h->rec[s];
     f.max_occupancy = h->d_max_occ;
     f.Nc = h->Nc; f.m = h->m; f.seed = h->seed; f.step = t;
     f.at_mode = at_mode; f.have_energy = have_energy ? 1 : 0;
     ProfScope prof(h, MPCD_PROF_FINALIZE);
     CUDA_TRY(h, cudaMemsetAsync(h->d_max_occ, 0, sizeof(int), h->stream));
-    cell_finalize<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(f);
+    cell_finalize<<<grid_for(h->Nc, 256 * kFinCells), 256, 0, h->stream>>>(f);
     LAUNCH_CHECK(h);
     if (zs) h->zeroed[o] = true;
     if (za) h->at_zeroed[o] = true;
@@ -289,19 +291,20 @@ int do_sort(mpcd_t *h, int s)
 
 inline bool sort_due(const mpcd_t *h, uint64_t t) { return h->opt.sort_period > 0 && (t % (uint64_t)h->opt.sort_period) == 0; }
 
-// bin + accumulate (+ finalize) for step t as a standalone block; energy always accumulated here
-int bin_accumulate(mpcd_t *h, uint64_t t, bool with_stream)
+// bin + accumulate + full finalize for step t as a standalone block; energy always accumulated here
+int bin_accumulate(mpcd_t *h, uint64_t t)
 {
     double s[3];
     draw_shift(h, t, s);
     if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) s[d] = (double)(float)s[d];   // A5
-    const int set = h->ccur;
+    const int set = (int)(t & 1);
     int rc = zero_set(h, set, true, false);
     if (rc) return rc;
     h->zeroed[set] = false;
-    rc = pass(h, (with_stream ? kStream : 0u) | kBin | kEnergy, set, t, t, s, h->opt.alpha);
+    rc = pass(h, kBin | kEnergy, set, set, t, t, s, h->opt.alpha);
     if (rc) return rc;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = s[d];
+    h->ccur = set;
     h->bin_valid = true; h->bin_step = t;
     rc = finalize(h, set, t, 0, true, false);
     if (rc) return rc;
@@ -416,7 +419,7 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
         if (!rc) rc = dev_alloc_t(h, &h->acc[s], (size_t)h->Nc * 4);
         if (!rc) rc = dev_alloc_t(h, &h->cnt[s], (size_t)h->Nc);
     }
-    if (!rc) rc = dev_alloc_t(h, &h->rec, (size_t)h->Nc);
+    for (int s = 0; s < 2 && !rc; ++s) rc = dev_alloc_t(h, &h->rec[s], (size_t)h->Nc);
     if (!rc) rc = dev_alloc_t(h, &h->cell_start, (size_t)h->Nc + 1);
     if (!rc) rc = dev_alloc_t(h, &h->tile_sum, (size_t)((h->Nc + kScanTile - 1) / kScanTile) + 1);
     if (!rc) rc = dev_alloc_t(h, &h->d_max_occ, 64);
@@ -448,7 +451,7 @@ int mpcd_stream(mpcd_t *h)
 {
     if (!h) return MPCD_EINVAL;
     const double zero[3] = {0, 0, 0};
-    int rc = pass(h, kStream, h->ccur, h->step, h->step, zero, h->opt.alpha);
+    int rc = pass(h, kStream, h->ccur, h->ccur, h->step, h->step, zero, h->opt.alpha);
     if (rc) return rc;
     h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
     return MPCD_OK;
@@ -457,7 +460,7 @@ int mpcd_stream(mpcd_t *h)
 int mpcd_shift_and_bin(mpcd_t *h)
 {
     if (!h) return MPCD_EINVAL;
-    return bin_accumulate(h, h->step, false);
+    return bin_accumulate(h, h->step);
 }
 
 int mpcd_collide_srd(mpcd_t *h, double alpha)
@@ -465,11 +468,12 @@ int mpcd_collide_srd(mpcd_t *h, double alpha)
     if (!h) return MPCD_EINVAL;
     if (!(h->bin_valid && h->bin_step == h->step && h->sums_valid && h->rec_valid))
         return fail(h, MPCD_ESTATE, "collide_srd needs mpcd_shift_and_bin for the current step first%s");
+    const int set = h->ccur;
     if (h->rec_mode != 0) {
-        int rc = finalize(h, h->ccur, h->step, 0, h->energy_valid, false);
+        int rc = finalize(h, set, h->step, 0, h->energy_valid, false);
         if (rc) return rc;
     }
-    int rc = pass(h, kSRD, h->ccur, h->step, h->step, h->shift_used, alpha);
+    int rc = pass(h, kSRD, set, set, h->step, h->step, h->shift_used, alpha);
     if (rc) return rc;
     h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
     return MPCD_OK;
@@ -486,9 +490,9 @@ int mpcd_collide_at(mpcd_t *h)
     rc = zero_set(h, set, false, true);
     if (rc) return rc;
     h->at_zeroed[set] = false;
-    rc = pass(h, kATDraw, set, h->step, h->step, h->shift_used, h->opt.alpha);       // second reduction
+    rc = pass(h, kATDraw, set, set, h->step, h->step, h->shift_used, h->opt.alpha);       // second reduction
     if (!rc) rc = finalize(h, set, h->step, 1, h->energy_valid, false);
-    if (!rc) rc = pass(h, kATApply, set, h->step, h->step, h->shift_used, h->opt.alpha);
+    if (!rc) rc = pass(h, kATApply, set, set, h->step, h->step, h->shift_used, h->opt.alpha);
     if (rc) return rc;
     h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
     return MPCD_OK;
@@ -518,13 +522,14 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
         draw_shift(h, step, s);
         if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) s[d] = (double)(float)s[d];
     };
+    // accumulator set and record set of step k are k & 1
     // first block: stream + bin + accumulate for step t
-    int set = h->ccur;
+    int set = (int)(t & 1);
     rc = zero_set(h, set, true, at);
     if (rc) return rc;
     shift_for(t);
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
-    rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), set, t, t, s, alpha);
+    rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), set, set, t, t, s, alpha);
     if (rc) return rc;
     if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
     rc = finalize(h, set, t, at ? 1 : 0, energy, nsteps > 1);
@@ -532,11 +537,11 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     // steady state: collide(t) fused with stream + bin + accumulate (t + 1): one pass per step
     for (int32_t j = 1; j < nsteps; ++j) {
         const int nxt = set ^ 1;
-        rc = zero_set(h, nxt, true, at);            // no-op when finalize already zeroed it
+        rc = zero_set(h, nxt, true, at);            // no-op: the previous finalize zeroed it
         if (rc) return rc;
         shift_for(t + 1);
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
-        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe, nxt, t, t + 1, s, alpha);
+        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe, set, nxt, t, t + 1, s, alpha);
         if (rc) return rc;
         set = nxt; t += 1;
         if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
@@ -544,7 +549,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
         if (rc) return rc;
     }
     // last collision
-    rc = pass(h, at ? kATApply : kSRD, set, t, t, s, alpha);
+    rc = pass(h, at ? kATApply : kSRD, set, set, t, t, s, alpha);
     if (rc) return rc;
     h->ccur = set;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = s[d];
@@ -605,7 +610,7 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
     double *d_ax = d_u + 3 * Nc;
     double *d_kT = d_ax + 3 * Nc;
     int32_t *d_cnt = reinterpret_cast<int32_t *>(d_kT + Nc);
-    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->cnt[h->ccur], h->rec, h->Nc, h->m, d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
+    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->cnt[h->ccur], h->rec[h->ccur], h->Nc, h->m, d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
     h->launches += 1;
     int rc = MPCD_OK;
     auto cp = [&](void *dst, const void *src, size_t b) {
@@ -629,7 +634,7 @@ int mpcd_get_thermo(mpcd_t *h, double P[3], double *KE, double *kT)
 {
     if (!h) return MPCD_EINVAL;
     if (!(h->sums_valid && h->energy_valid)) {
-        int rc = bin_accumulate(h, h->bin_valid ? h->bin_step : h->step, false);
+        int rc = bin_accumulate(h, h->bin_valid ? h->bin_step : h->step);
         if (rc) return rc;
     }
     CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, 8 * sizeof(double), h->stream));

@@ -103,6 +103,25 @@ __device__ __forceinline__ void store4(double4 *p, double4 v)
     reinterpret_cast<double2 *>(p)[1] = double2{v.z, v.w};
 }
 
+// 32-byte (one full sector) accesses for the per-cell records: sm_100 has 256-bit LDG/STG.
+struct f64x4 { double x, y, z, w; };
+__device__ __forceinline__ f64x4 ld256_nc(const double *p)     // read-only path
+{
+    f64x4 r;
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ f64x4 ld256(const double *p)
+{
+    f64x4 r;
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.w) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st256(double *p, double a, double b, double c, double d)
+{
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" :: "l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
 // eq. 1 PAPER.md:35 + periodic wrap (A7): x = fl(x + fl(v dt)); if x < 0: x += L; if x >= L: x -= L.
 template <typename T> __device__ __forceinline__ T stream_wrap(T x, T v, T dt, T L)
 {

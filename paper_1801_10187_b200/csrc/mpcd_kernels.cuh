@@ -65,9 +65,10 @@ __global__ void __launch_bounds__(kPassThreads) particle_pass(const PassArgs<T> 
     if (F & kSRD) {
         if (valid) {
             // Alg. 1 lines 2-4: gather the cell's mean velocity and axis (3 x 16 B of one 64-B record)
-            const double2 *r = reinterpret_cast<const double2 *>(a.rec + c);
-            const double2 r0 = __ldg(r), r1 = __ldg(r + 1), r2 = __ldg(r + 2);
-            const double ux = r0.x, uy = r0.y, uz = r1.x, nx = r1.y, ny = r2.x, nz = r2.y;
+            const double *r = reinterpret_cast<const double *>(a.rec + c);
+            const f64x4 r0 = ld256_nc(r);                                    // one full sector
+            const double2 r2 = __ldg(reinterpret_cast<const double2 *>(r + 4));
+            const double ux = r0.x, uy = r0.y, uz = r0.z, nx = r0.w, ny = r2.x, nz = r2.y;
             const double wx = (double)v.x - ux, wy = (double)v.y - uy, wz = (double)v.z - uz;   // lines 5-6
             const double ndw = nx * wx + ny * wy + nz * wz;                                    // line 7
             const double omc = 1.0 - a.cos_a;
@@ -82,8 +83,8 @@ __global__ void __launch_bounds__(kPassThreads) particle_pass(const PassArgs<T> 
         if (valid) {
             double g0, g1, g2;
             draw_gauss3(a.seed, a.step_collide, tag, g0, g1, g2);
-            const double2 *r = reinterpret_cast<const double2 *>(a.rec + c);
-            const double2 r1 = __ldg(r + 1), r2 = __ldg(r + 2);     // r[] = u - D/N_c
+            const double *r = reinterpret_cast<const double *>(a.rec + c);               // r[] = u - D/N_c
+            const double2 r1 = __ldg(reinterpret_cast<const double2 *>(r + 2)), r2 = __ldg(reinterpret_cast<const double2 *>(r + 4));
             v.x = (T)(r1.y + a.sigma * g0); v.y = (T)(r2.x + a.sigma * g1); v.z = (T)(r2.y + a.sigma * g2);
             v.w = T(0);
             store4(a.vel + i, v);
@@ -124,50 +125,60 @@ __global__ void __launch_bounds__(kPassThreads) particle_pass(const PassArgs<T> 
 // ---------------------------------------------------------------------------------------
 struct FinalizeArgs {
     const double *acc; const int32_t *cnt; const double *at_acc;   // this step
-    double *acc_next; int32_t *cnt_next; double *at_acc_next;      // zeroed for the next step
+    double *acc_next; int32_t *cnt_next; double *at_acc_next;      // zeroed for the next step (may be NULL)
     CellRec *rec;
     int *max_occupancy;
     int64_t Nc;
     double m;
     uint64_t seed, step;
-    int at_mode;     // 0: r = axis; 1: r = u - D/N_c
+    int at_mode;      // 0: r = axis; 1: r = u - D/N_c
     int have_energy;
 };
 
-__global__ void __launch_bounds__(256) cell_finalize(const FinalizeArgs a)
+constexpr int kFinCells = 2;     // cells per thread: all loads are issued before any is used (memory-level parallelism)
+
+__global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
 {
-    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    int n = 0;
-    if (c < a.Nc) {
-        const double2 s0 = reinterpret_cast<const double2 *>(a.acc + 4 * c)[0];
-        const double2 s1 = reinterpret_cast<const double2 *>(a.acc + 4 * c)[1];
-        n = a.cnt[c];
-        CellRec r;
-        const double dn = (double)n;
-        r.u[0] = n > 0 ? s0.x / dn : 0.0;
-        r.u[1] = n > 0 ? s0.y / dn : 0.0;
-        r.u[2] = n > 0 ? s1.x / dn : 0.0;
-        double kT = 0.0;
-        if (a.have_energy && n >= 2) {
-            const double erel = 0.5 * a.m * (s1.y - dn * (r.u[0] * r.u[0] + r.u[1] * r.u[1] + r.u[2] * r.u[2]));
-            kT = 2.0 * erel / (3.0 * (double)(n - 1));
+    const int64_t c0 = (int64_t)blockIdx.x * (256 * kFinCells) + threadIdx.x;
+    double2 s0[kFinCells], s1[kFinCells], d0[kFinCells], d1[kFinCells];
+    int n[kFinCells];
+#pragma unroll
+    for (int k = 0; k < kFinCells; ++k) {
+        const int64_t c = c0 + 256 * k;
+        n[k] = 0;
+        if (c < a.Nc) {
+            s0[k] = reinterpret_cast<const double2 *>(a.acc + 4 * c)[0];
+            s1[k] = reinterpret_cast<const double2 *>(a.acc + 4 * c)[1];
+            n[k] = a.cnt[c];
+            if (a.at_mode) {
+                d0[k] = reinterpret_cast<const double2 *>(a.at_acc + 4 * c)[0];
+                d1[k] = reinterpret_cast<const double2 *>(a.at_acc + 4 * c)[1];
+            }
         }
-        r.kT = kT;
-        r.count = n;
+    }
+    int nmax = 0;
+#pragma unroll
+    for (int k = 0; k < kFinCells; ++k) {
+        const int64_t c = c0 + 256 * k;
+        if (c >= a.Nc) continue;
+        const double dn = (double)n[k];
+        double u[3] = {0, 0, 0}, kT = 0.0;
+        if (n[k] > 0) { u[0] = s0[k].x / dn; u[1] = s0[k].y / dn; u[2] = s1[k].x / dn; }
+        if (a.have_energy && n[k] >= 2) {
+            const double erel = 0.5 * a.m * (s1[k].y - dn * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
+            kT = 2.0 * erel / (3.0 * (double)(n[k] - 1));
+        }
+        double r[3] = {0, 0, 0};
         if (a.at_mode) {
-            const double2 d0 = reinterpret_cast<const double2 *>(a.at_acc + 4 * c)[0];
-            const double2 d1 = reinterpret_cast<const double2 *>(a.at_acc + 4 * c)[1];
-            r.r[0] = n > 0 ? r.u[0] - d0.x / dn : 0.0;
-            r.r[1] = n > 0 ? r.u[1] - d0.y / dn : 0.0;
-            r.r[2] = n > 0 ? r.u[2] - d1.x / dn : 0.0;
+            if (n[k] > 0) { r[0] = u[0] - d0[k].x / dn; r[1] = u[1] - d0[k].y / dn; r[2] = u[2] - d1[k].x / dn; }
         } else {
-            draw_axis(a.seed, a.step, (uint32_t)c, r.r[0], r.r[1], r.r[2]);
+            draw_axis(a.seed, a.step, (uint32_t)c, r[0], r[1], r[2]);
         }
         double2 *out = reinterpret_cast<double2 *>(a.rec + c);
-        out[0] = double2{r.u[0], r.u[1]};
-        out[1] = double2{r.u[2], r.r[0]};
-        out[2] = double2{r.r[1], r.r[2]};
-        out[3] = double2{r.kT, __longlong_as_double(r.count)};
+        out[0] = double2{u[0], u[1]};
+        out[1] = double2{u[2], r[0]};
+        out[2] = double2{r[1], r[2]};
+        out[3] = double2{kT, __longlong_as_double((long long)n[k])};
         if (a.acc_next) {
             reinterpret_cast<double2 *>(a.acc_next + 4 * c)[0] = double2{0.0, 0.0};
             reinterpret_cast<double2 *>(a.acc_next + 4 * c)[1] = double2{0.0, 0.0};
@@ -177,8 +188,9 @@ __global__ void __launch_bounds__(256) cell_finalize(const FinalizeArgs a)
             reinterpret_cast<double2 *>(a.at_acc_next + 4 * c)[0] = double2{0.0, 0.0};
             reinterpret_cast<double2 *>(a.at_acc_next + 4 * c)[1] = double2{0.0, 0.0};
         }
+        nmax = n[k] > nmax ? n[k] : nmax;
     }
-    const int wmax = __reduce_max_sync(0xffffffffu, n);
+    const int wmax = __reduce_max_sync(0xffffffffu, nmax);
     if ((threadIdx.x & 31) == 0 && wmax > 0) atomicMax(a.max_occupancy, wmax);
 }
 
