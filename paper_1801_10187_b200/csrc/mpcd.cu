@@ -38,7 +38,7 @@ struct mpcd {
     int pcur = 0;
     // cell arrays
     double *acc[2] = {nullptr, nullptr};
-    int32_t *cnt[2] = {nullptr, nullptr};
+    double *qacc[2] = {nullptr, nullptr};
     double *at_acc[2] = {nullptr, nullptr};
     CellRec *rec[2] = {nullptr, nullptr};   // per accumulator set (step parity)
     int32_t *cell_start = nullptr, *tile_sum = nullptr;
@@ -156,7 +156,7 @@ template <typename T> PassArgs<T> make_args(mpcd_t *h, int rec_set, int acc_set,
     a.cell = h->cell[h->pcur];
     a.rec = h->rec[rec_set];
     a.acc = h->acc[acc_set];
-    a.cnt = h->cnt[acc_set];
+    a.qacc = h->qacc[acc_set];
     a.at_acc = h->at_acc[acc_set];
     a.N = h->N;
     for (int d = 0; d < 3; ++d) {
@@ -230,7 +230,7 @@ int zero_set(mpcd_t *h, int s, bool sums, bool at)
     sums = sums && !h->zeroed[s];
     at = at && h->at_acc[s] && !h->at_zeroed[s];
     if (!sums && !at) return MPCD_OK;
-    cell_zero<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(sums ? h->acc[s] : nullptr, h->cnt[s], at ? h->at_acc[s] : nullptr, h->Nc);
+    cell_zero<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(sums ? h->acc[s] : nullptr, h->qacc[s], at ? h->at_acc[s] : nullptr, h->Nc);
     LAUNCH_CHECK(h);
     if (sums) h->zeroed[s] = true;
     if (at) h->at_zeroed[s] = true;
@@ -241,12 +241,12 @@ int zero_set(mpcd_t *h, int s, bool sums, bool at)
 int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool zero_next)
 {
     FinalizeArgs f{};
-    f.acc = h->acc[s]; f.cnt = h->cnt[s]; f.at_acc = h->at_acc[s];
+    f.acc = h->acc[s]; f.qacc = h->qacc[s]; f.at_acc = h->at_acc[s];
     const int o = s ^ 1;
     const bool zs = zero_next && !h->zeroed[o];
     const bool za = zero_next && h->at_acc[o] && !h->at_zeroed[o] && at_mode;
     f.acc_next = zs ? h->acc[o] : nullptr;
-    f.cnt_next = zs ? h->cnt[o] : nullptr;
+    f.qacc_next = zs ? h->qacc[o] : nullptr;
     f.at_acc_next = za ? h->at_acc[o] : nullptr;
     f.rec = h->rec[s];
     f.max_occupancy = h->d_max_occ;
@@ -268,11 +268,11 @@ int do_sort(mpcd_t *h, int s)
 {
     const int ntiles = (int)((h->Nc + kScanTile - 1) / kScanTile);
     ProfScope prof(h, MPCD_PROF_SORT);
-    scan_tile_sums<<<ntiles, kScanThreads, 0, h->stream>>>(h->cnt[s], h->Nc, h->tile_sum);
+    scan_tile_sums<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum);
     LAUNCH_CHECK(h);
     scan_tile_offsets<<<1, 1024, 0, h->stream>>>(h->tile_sum, ntiles);
     LAUNCH_CHECK(h);
-    scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->cnt[s], h->Nc, h->tile_sum, h->cell_start);
+    scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum, h->cell_start);
     LAUNCH_CHECK(h);
     const int src = h->pcur, dst = src ^ 1;
     if (h->opt.precision == MPCD_FP64)
@@ -417,7 +417,7 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
         if (!rc) rc = dev_alloc_t(h, &h->tag[s], (size_t)N);
         if (!rc) rc = dev_alloc_t(h, &h->cell[s], (size_t)N);
         if (!rc) rc = dev_alloc_t(h, &h->acc[s], (size_t)h->Nc * 4);
-        if (!rc) rc = dev_alloc_t(h, &h->cnt[s], (size_t)h->Nc);
+        if (!rc) rc = dev_alloc_t(h, &h->qacc[s], (size_t)h->Nc);
     }
     for (int s = 0; s < 2 && !rc; ++s) rc = dev_alloc_t(h, &h->rec[s], (size_t)h->Nc);
     if (!rc) rc = dev_alloc_t(h, &h->cell_start, (size_t)h->Nc + 1);
@@ -610,7 +610,7 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
     double *d_ax = d_u + 3 * Nc;
     double *d_kT = d_ax + 3 * Nc;
     int32_t *d_cnt = reinterpret_cast<int32_t *>(d_kT + Nc);
-    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->cnt[h->ccur], h->rec[h->ccur], h->Nc, h->m, d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
+    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->rec[h->ccur], h->Nc, h->m, d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
     h->launches += 1;
     int rc = MPCD_OK;
     auto cp = [&](void *dst, const void *src, size_t b) {
@@ -638,7 +638,7 @@ int mpcd_get_thermo(mpcd_t *h, double P[3], double *KE, double *kT)
         if (rc) return rc;
     }
     CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, 8 * sizeof(double), h->stream));
-    cell_thermo<<<148 * 4, 256, 0, h->stream>>>(h->acc[h->ccur], h->cnt[h->ccur], h->Nc, h->m, h->d_scalars);
+    cell_thermo<<<148 * 4, 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->Nc, h->m, h->d_scalars);
     LAUNCH_CHECK(h);
     double out[6];
     CUDA_TRY(h, cudaMemcpyAsync(out, h->d_scalars, sizeof(out), cudaMemcpyDeviceToHost, h->stream));

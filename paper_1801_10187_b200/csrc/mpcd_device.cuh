@@ -141,24 +141,26 @@ template <typename T> __device__ __forceinline__ int bin_axis(T x, T s, T inv_a,
 }
 
 // ---------------------------------------------------------------------------------------
-// Per-cell fp64 accumulation.  Layout in HBM: acc[c] = {Sx, Sy, Sz, Q}
-// (4 doubles = one 32-byte sector, Q = sum |v|^2) and cnt[c] (int32).
+// Per-cell fp64 accumulation.  Layout in HBM: acc[c] = {Sx, Sy, Sz, N}
+// (4 doubles = one 32-byte sector; the count N is kept as a double, exact below 2^53) and,
+// when the kinetic energy is wanted, q[c] = sum |v|^2 in an array of its own.
 //
-// The L2 atomic path of a B200 SM retires about one RED *request* (distinct 32-byte sector
-// per instruction) every ~1.3 cycles, which -- not HBM bandwidth -- bounds this step
-// (profiles/r01_atomics_probe.md).  So lanes are first combined by cell inside the warp
-// (match.any + shuffle tree), and the surviving leaders are then issued "transposed": four
-// adjacent lanes add the four doubles of ONE record in one instruction, i.e. one sector
-// request per (leader, record) instead of four.
+// What bounds this step on a B200 is not HBM bandwidth but the L1/LSU data pipe: about one
+// "wavefront" per cycle per SM, and a RED costs one per distinct 32-byte sector per
+// instruction (profiles/r01_*.md).  So lanes are first combined by cell inside the warp
+// (match.any + a shuffle tree, ~2.3 particles per surviving leader on the benchmark fluid),
+// and the leaders are then issued "transposed": four adjacent lanes add the four doubles of
+// ONE record in one instruction -- one sector request per leader instead of four.
 // ---------------------------------------------------------------------------------------
-struct WarpScratch {           // per-warp staging for the transposed issue
-    double v[32][4];
+constexpr int kStagePitch = 36;    // doubles per staged component row: 4 rows land in disjoint banks for one half-warp
+struct WarpScratch {               // per-warp staging for the transposed issue
+    double v[4][kStagePitch];      // [component][leader]
+    double q[32];
     int cell[32];
-    int n[32];
 };
 
-template <bool kEnergy>
-__device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, int *__restrict__ cnt, WarpScratch &ws,
+template <bool kCount, bool kEnergy>
+__device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, double *__restrict__ qacc, WarpScratch &ws,
                                                      int c /* < 0 = inactive lane, unique per lane */, double vx, double vy, double vz)
 {
     const unsigned full = 0xffffffffu;
@@ -182,52 +184,18 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, i
     const int nl = __popc(leaders);
     if (leader && c >= 0) {
         const int j = __popc(leaders & ((1u << lane) - 1u));
-        ws.v[j][0] = vx; ws.v[j][1] = vy; ws.v[j][2] = vz; ws.v[j][3] = q;
-        ws.cell[j] = c; ws.n[j] = size;
-    }
-    __syncwarp();
-    const int comp = lane & 3;
-    for (int base = 0; base < nl; base += 8) {
-        const int j = base + (lane >> 2);
-        if (j < nl) {
-            const int cc = ws.cell[j];
-            if (kEnergy || comp < 3) atomicAdd(acc + 4 * (size_t)cc + comp, ws.v[j][comp]);
-            if (comp == 0) atomicAdd(cnt + cc, ws.n[j]);
-        }
-    }
-    __syncwarp();
-}
-
-// Same for a 3-vector only (the Andersen-thermostat second reduction).
-__device__ __forceinline__ void warp_cell_accumulate3(double *__restrict__ acc, WarpScratch &ws, int c, double vx, double vy, double vz)
-{
-    const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    unsigned peers = __match_any_sync(full, c);
-    const bool leader = (__ffs(peers) - 1) == lane;
-    int rank = __popc(peers & ((1u << lane) - 1u));
-    peers &= (0xfffffffeu << lane);
-    while (__any_sync(full, peers != 0u)) {
-        const int next = __ffs(peers);
-        const int src = next ? next - 1 : lane;
-        const double tx = __shfl_sync(full, vx, src), ty = __shfl_sync(full, vy, src), tz = __shfl_sync(full, vz, src);
-        if (next) { vx += tx; vy += ty; vz += tz; }
-        peers &= __ballot_sync(full, !(rank & 1));
-        rank >>= 1;
-    }
-    const unsigned leaders = __ballot_sync(full, leader && c >= 0);
-    const int nl = __popc(leaders);
-    if (leader && c >= 0) {
-        const int j = __popc(leaders & ((1u << lane) - 1u));
-        ws.v[j][0] = vx; ws.v[j][1] = vy; ws.v[j][2] = vz;
+        ws.v[0][j] = vx; ws.v[1][j] = vy; ws.v[2][j] = vz;
+        if (kCount) ws.v[3][j] = (double)size;
+        if (kEnergy) ws.q[j] = q;
         ws.cell[j] = c;
     }
     __syncwarp();
     const int comp = lane & 3;
     for (int base = 0; base < nl; base += 8) {
         const int j = base + (lane >> 2);
-        if (j < nl && comp < 3) atomicAdd(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[j][comp]);
+        if (j < nl && (kCount || comp < 3)) atomicAdd(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[comp][j]);
     }
+    if (kEnergy && lane < nl) atomicAdd(qacc + ws.cell[lane], ws.q[lane]);
     __syncwarp();
 }
 

@@ -34,8 +34,8 @@ template <typename T> struct PassArgs {
     uint32_t *tag;
     int32_t *cell;
     const CellRec *rec;   // results of the step being collided
-    double *acc;          // accumulators of the step being binned: {Sx, Sy, Sz, Q} per cell
-    int32_t *cnt;
+    double *acc;          // accumulators of the step being binned: {Sx, Sy, Sz, N} per cell
+    double *qacc;         // sum |v|^2 per cell (kEnergy)
     double *at_acc;       // {Dx, Dy, Dz, -} per cell (AT second reduction)
     int64_t N;
     int32_t n[3];
@@ -107,14 +107,14 @@ __global__ void __launch_bounds__(kPassThreads) particle_pass(const PassArgs<T> 
             c2 = ix + a.n[0] * (iy + a.n[1] * iz);                    // A8
             a.cell[i] = c2;
         }
-        warp_cell_accumulate<(F & kEnergy) != 0>(a.acc, a.cnt, ws[threadIdx.x >> 5], c2, (double)v.x, (double)v.y, (double)v.z);
+        warp_cell_accumulate<true, (F & kEnergy) != 0>(a.acc, a.qacc, ws[threadIdx.x >> 5], c2, (double)v.x, (double)v.y, (double)v.z);
         c = c2;
     }
     if (F & kATDraw) {
         double g0 = 0, g1 = 0, g2 = 0;
         if (valid) draw_gauss3(a.seed, a.step_bin, tag, g0, g1, g2);
-        warp_cell_accumulate3(a.at_acc, ws[threadIdx.x >> 5], valid ? c : -1 - (int)(threadIdx.x & 31),
-                              a.sigma * g0, a.sigma * g1, a.sigma * g2);
+        warp_cell_accumulate<false, false>(a.at_acc, nullptr, ws[threadIdx.x >> 5], valid ? c : -1 - (int)(threadIdx.x & 31),
+                                           a.sigma * g0, a.sigma * g1, a.sigma * g2);
     }
 }
 
@@ -124,8 +124,8 @@ __global__ void __launch_bounds__(kPassThreads) particle_pass(const PassArgs<T> 
 // and zeroes the OTHER accumulator set so the next step can accumulate into it.
 // ---------------------------------------------------------------------------------------
 struct FinalizeArgs {
-    const double *acc; const int32_t *cnt; const double *at_acc;   // this step
-    double *acc_next; int32_t *cnt_next; double *at_acc_next;      // zeroed for the next step (may be NULL)
+    const double *acc; const double *qacc; const double *at_acc;   // this step
+    double *acc_next; double *qacc_next; double *at_acc_next;      // zeroed for the next step (may be NULL)
     CellRec *rec;
     int *max_occupancy;
     int64_t Nc;
@@ -141,6 +141,7 @@ __global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
 {
     const int64_t c0 = (int64_t)blockIdx.x * (256 * kFinCells) + threadIdx.x;
     double2 s0[kFinCells], s1[kFinCells], d0[kFinCells], d1[kFinCells];
+    double qq[kFinCells];
     int n[kFinCells];
 #pragma unroll
     for (int k = 0; k < kFinCells; ++k) {
@@ -149,7 +150,7 @@ __global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
         if (c < a.Nc) {
             s0[k] = reinterpret_cast<const double2 *>(a.acc + 4 * c)[0];
             s1[k] = reinterpret_cast<const double2 *>(a.acc + 4 * c)[1];
-            n[k] = a.cnt[c];
+            qq[k] = a.have_energy ? a.qacc[c] : 0.0;
             if (a.at_mode) {
                 d0[k] = reinterpret_cast<const double2 *>(a.at_acc + 4 * c)[0];
                 d1[k] = reinterpret_cast<const double2 *>(a.at_acc + 4 * c)[1];
@@ -161,11 +162,12 @@ __global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
     for (int k = 0; k < kFinCells; ++k) {
         const int64_t c = c0 + 256 * k;
         if (c >= a.Nc) continue;
-        const double dn = (double)n[k];
+        const double dn = s1[k].y;
+        n[k] = (int)dn;
         double u[3] = {0, 0, 0}, kT = 0.0;
         if (n[k] > 0) { u[0] = s0[k].x / dn; u[1] = s0[k].y / dn; u[2] = s1[k].x / dn; }
         if (a.have_energy && n[k] >= 2) {
-            const double erel = 0.5 * a.m * (s1[k].y - dn * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
+            const double erel = 0.5 * a.m * (qq[k] - dn * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
             kT = 2.0 * erel / (3.0 * (double)(n[k] - 1));
         }
         double r[3] = {0, 0, 0};
@@ -182,7 +184,7 @@ __global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
         if (a.acc_next) {
             reinterpret_cast<double2 *>(a.acc_next + 4 * c)[0] = double2{0.0, 0.0};
             reinterpret_cast<double2 *>(a.acc_next + 4 * c)[1] = double2{0.0, 0.0};
-            a.cnt_next[c] = 0;
+            if (a.qacc_next) a.qacc_next[c] = 0.0;
         }
         if (a.at_acc_next) {
             reinterpret_cast<double2 *>(a.at_acc_next + 4 * c)[0] = double2{0.0, 0.0};
@@ -195,14 +197,14 @@ __global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
 }
 
 // zero one accumulator set
-__global__ void __launch_bounds__(256) cell_zero(double *acc, int32_t *cnt, double *at_acc, int64_t Nc)
+__global__ void __launch_bounds__(256) cell_zero(double *acc, double *qacc, double *at_acc, int64_t Nc)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
     if (acc) {
         reinterpret_cast<double2 *>(acc + 4 * c)[0] = double2{0.0, 0.0};
         reinterpret_cast<double2 *>(acc + 4 * c)[1] = double2{0.0, 0.0};
-        cnt[c] = 0;
+        qacc[c] = 0.0;
     }
     if (at_acc) {
         reinterpret_cast<double2 *>(at_acc + 4 * c)[0] = double2{0.0, 0.0};
@@ -212,17 +214,16 @@ __global__ void __launch_bounds__(256) cell_zero(double *acc, int32_t *cnt, doub
 
 // a9. Net momentum, kinetic energy, pooled temperature by device-wide reduction.
 // out = {sum Sx, sum Sy, sum Sz, sum Q, sum E_rel over N_c >= 2, sum 1.5 (N_c - 1)}
-__global__ void __launch_bounds__(256) cell_thermo(const double *acc, const int32_t *cnt, int64_t Nc, double m, double *out)
+__global__ void __launch_bounds__(256) cell_thermo(const double *acc, const double *qacc, int64_t Nc, double m, double *out)
 {
     double v[6] = {0, 0, 0, 0, 0, 0};
     for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c < Nc; c += (int64_t)gridDim.x * blockDim.x) {
         const double2 s0 = reinterpret_cast<const double2 *>(acc + 4 * c)[0];
         const double2 s1 = reinterpret_cast<const double2 *>(acc + 4 * c)[1];
-        const int n = cnt[c];
-        v[0] += s0.x; v[1] += s0.y; v[2] += s1.x; v[3] += s1.y;
-        if (n >= 2) {
-            const double dn = (double)n;
-            v[4] += 0.5 * m * (s1.y - (s0.x * s0.x + s0.y * s0.y + s1.x * s1.x) / dn);
+        const double q = qacc[c], dn = s1.y;
+        v[0] += s0.x; v[1] += s0.y; v[2] += s1.x; v[3] += q;
+        if (dn >= 2.0) {
+            v[4] += 0.5 * m * (q - (s0.x * s0.x + s0.y * s0.y + s1.x * s1.x) / dn);
             v[5] += 1.5 * (dn - 1.0);
         }
     }
@@ -230,14 +231,14 @@ __global__ void __launch_bounds__(256) cell_thermo(const double *acc, const int3
 }
 
 // Unpack the cell arrays for mpcd_get_cells (SoA outputs on the device, copied by the host).
-__global__ void __launch_bounds__(256) cell_unpack(const double *acc, const int32_t *cnt, const CellRec *rec, int64_t Nc, double m,
+__global__ void __launch_bounds__(256) cell_unpack(const double *acc, const double *qacc, const CellRec *rec, int64_t Nc, double m,
                                                    int32_t *count, double *sumv3, double *ke, double *u3, double *axis3, double *kTc)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
-    if (count) count[c] = cnt[c];
+    if (count) count[c] = (int32_t)acc[4 * c + 3];
     if (sumv3) { sumv3[3 * c] = acc[4 * c]; sumv3[3 * c + 1] = acc[4 * c + 1]; sumv3[3 * c + 2] = acc[4 * c + 2]; }
-    if (ke) ke[c] = 0.5 * m * acc[4 * c + 3];
+    if (ke) ke[c] = 0.5 * m * qacc[c];
     if (u3) { u3[3 * c] = rec[c].u[0]; u3[3 * c + 1] = rec[c].u[1]; u3[3 * c + 2] = rec[c].u[2]; }
     if (axis3) { axis3[3 * c] = rec[c].r[0]; axis3[3 * c + 1] = rec[c].r[1]; axis3[3 * c + 2] = rec[c].r[2]; }
     if (kTc) kTc[c] = rec[c].kT;
@@ -250,14 +251,14 @@ __global__ void __launch_bounds__(256) cell_unpack(const double *acc, const int3
 // ---------------------------------------------------------------------------------------
 constexpr int kScanThreads = 256, kScanItems = 16, kScanTile = kScanThreads * kScanItems;
 
-__global__ void __launch_bounds__(kScanThreads) scan_tile_sums(const int32_t *cnt, int64_t Nc, int32_t *tile_sum)
+__global__ void __launch_bounds__(kScanThreads) scan_tile_sums(const double *acc, int64_t Nc, int32_t *tile_sum)
 {
     __shared__ int sm[kScanThreads / 32];
     const int64_t base = (int64_t)blockIdx.x * kScanTile;
     int s = 0;
     for (int k = 0; k < kScanItems; ++k) {
         const int64_t c = base + (int64_t)k * kScanThreads + threadIdx.x;
-        if (c < Nc) s += cnt[c];
+        if (c < Nc) s += (int)acc[4 * c + 3];
     }
     s = __reduce_add_sync(0xffffffffu, s);
     if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
@@ -295,7 +296,7 @@ __global__ void __launch_bounds__(1024) scan_tile_offsets(int32_t *tile_sum, int
     }
 }
 
-__global__ void __launch_bounds__(kScanThreads) scan_cells(const int32_t *cnt, int64_t Nc, const int32_t *tile_off, int32_t *cell_start)
+__global__ void __launch_bounds__(kScanThreads) scan_cells(const double *acc, int64_t Nc, const int32_t *tile_off, int32_t *cell_start)
 {
     // thread t owns kScanItems consecutive cells of the tile
     __shared__ int sm[kScanThreads];
@@ -303,7 +304,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_cells(const int32_t *cnt, i
     int x[kScanItems];
     int s = 0;
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) { x[k] = (base + k < Nc) ? cnt[base + k] : 0; s += x[k]; }
+    for (int k = 0; k < kScanItems; ++k) { x[k] = (base + k < Nc) ? (int)acc[4 * (base + k) + 3] : 0; s += x[k]; }
     sm[threadIdx.x] = s;
     __syncthreads();
     for (int o = 1; o < kScanThreads; o <<= 1) {
