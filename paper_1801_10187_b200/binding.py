@@ -14,7 +14,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmpcd_b200.so")
+LIB_PATH = os.environ.get("MPCD_B200_LIB") or os.path.join(_HERE, "libmpcd_b200.so")   # override: an alternative build of the same library
 
 MPCD_OK, MPCD_EINVAL, MPCD_ENOMEM, MPCD_ECUDA, MPCD_ESTATE = 0, -1, -2, -3, -4
 MPCD_MIXED, MPCD_FP64 = 0, 1

@@ -34,17 +34,18 @@ struct mpcd {
     // particle arrays, double-buffered for the sort
     void *pos[2] = {nullptr, nullptr}, *vel[2] = {nullptr, nullptr};
     uint32_t *tag[2] = {nullptr, nullptr};
-    int32_t *cell[2] = {nullptr, nullptr};
+    int32_t *cell = nullptr;       // cell index per particle, filled on demand only (mpcd_get_state / mpcd_device_ptrs)
     int pcur = 0;
     // cell arrays
     double *acc[2] = {nullptr, nullptr};
     double *qacc[2] = {nullptr, nullptr};
     double *at_acc[2] = {nullptr, nullptr};
-    CellRec *rec[2] = {nullptr, nullptr};   // per accumulator set (step parity)
+    double *rec[2] = {nullptr, nullptr};    // kRecDoubles per cell, per accumulator set (step parity)
     int32_t *cell_start = nullptr, *tile_sum = nullptr;
     int *d_max_occ = nullptr;
     double *d_scalars = nullptr;   // 8 doubles of scratch for reductions
     int ccur = 0;                  // accumulator set of the current bin
+    int64_t prefetch_blocks = 0;   // L2 prefetch distance of the particle pass, in blocks
     bool zeroed[2] = {false, false}, at_zeroed[2] = {false, false};
     // state machine
     uint64_t step = 0, bin_step = 0;
@@ -146,19 +147,19 @@ void draw_shift(const mpcd_t *h, uint64_t step, double s[3])
     for (int d = 0; d < 3; ++d) s[d] = (u01_32(w[d]) - 0.5) * h->a;
 }
 
-template <typename T> PassArgs<T> make_args(mpcd_t *h, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3],
-                                            double alpha)
+template <typename T> PassArgs<T> make_args(mpcd_t *h, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift_c[3],
+                                            const double shift[3], double alpha)
 {
     PassArgs<T> a{};
     a.pos = static_cast<typename Vec4<T>::type *>(h->pos[h->pcur]);
     a.vel = static_cast<typename Vec4<T>::type *>(h->vel[h->pcur]);
     a.tag = h->tag[h->pcur];
-    a.cell = h->cell[h->pcur];
     a.rec = h->rec[rec_set];
     a.acc = h->acc[acc_set];
     a.qacc = h->qacc[acc_set];
     a.at_acc = h->at_acc[acc_set];
     a.N = h->N;
+    a.prefetch = h->prefetch_blocks * (int64_t)kPassThreads;
     for (int d = 0; d < 3; ++d) {
         a.n[d] = h->n[d];
         a.L[d] = (T)h->box[d];
@@ -181,9 +182,9 @@ template <typename T, unsigned F> void launch_pass_t(mpcd_t *h, const PassArgs<T
 }
 
 template <typename T> int launch_pass(mpcd_t *h, unsigned F, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin,
-                                      const double shift[3], double alpha)
+                                      const double shift_c[3], const double shift[3], double alpha)
 {
-    const PassArgs<T> a = make_args<T>(h, rec_set, acc_set, step_collide, step_bin, shift, alpha);
+    const PassArgs<T> a = make_args<T>(h, rec_set, acc_set, step_collide, step_bin, shift_c, shift, alpha);
     switch (F) {
 #define CASE(f) case (f): launch_pass_t<T, (f)>(h, a); break;
         CASE(kStream)
@@ -206,12 +207,14 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, int rec_set, int ac
     return MPCD_OK;
 }
 
-int pass(mpcd_t *h, unsigned F, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift[3], double alpha)
+// shift_c: grid shift of the step being collided; shift: grid shift of the step being binned
+int pass(mpcd_t *h, unsigned F, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift_c[3], const double shift[3],
+         double alpha)
 {
     const bool collide = (F & (kSRD | kATApply)) != 0, bin = (F & kBin) != 0;
     ProfScope prof(h, collide && bin ? MPCD_PROF_FUSED : (collide ? MPCD_PROF_COLLIDE : (bin ? MPCD_PROF_BIN : MPCD_PROF_OTHER)));
-    return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, rec_set, acc_set, step_collide, step_bin, shift, alpha)
-                                         : launch_pass<float>(h, F, rec_set, acc_set, step_collide, step_bin, shift, alpha);
+    return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, rec_set, acc_set, step_collide, step_bin, shift_c, shift, alpha)
+                                         : launch_pass<float>(h, F, rec_set, acc_set, step_collide, step_bin, shift_c, shift, alpha);
 }
 
 int ensure_at_buffers(mpcd_t *h)
@@ -238,10 +241,10 @@ int zero_set(mpcd_t *h, int s, bool sums, bool at)
 }
 
 // a5 for accumulator set `s` at step `t` into rec[s]; optionally zero the other set for the next step.
-int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool zero_next)
+int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool zero_next)
 {
     FinalizeArgs f{};
-    f.acc = h->acc[s]; f.qacc = h->qacc[s]; f.at_acc = h->at_acc[s];
+    f.acc = h->acc[s]; f.at_acc = h->at_acc[s];
     const int o = s ^ 1;
     const bool zs = zero_next && !h->zeroed[o];
     const bool za = zero_next && h->at_acc[o] && !h->at_zeroed[o] && at_mode;
@@ -250,8 +253,8 @@ int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool z
     f.at_acc_next = za ? h->at_acc[o] : nullptr;
     f.rec = h->rec[s];
     f.max_occupancy = h->d_max_occ;
-    f.Nc = h->Nc; f.m = h->m; f.seed = h->seed; f.step = t;
-    f.at_mode = at_mode; f.have_energy = have_energy ? 1 : 0;
+    f.Nc = h->Nc; f.seed = h->seed; f.step = t;
+    f.at_mode = at_mode;
     ProfScope prof(h, MPCD_PROF_FINALIZE);
     CUDA_TRY(h, cudaMemsetAsync(h->d_max_occ, 0, sizeof(int), h->stream));
     cell_finalize<<<grid_for(h->Nc, 256 * kFinCells), 256, 0, h->stream>>>(f);
@@ -263,8 +266,9 @@ int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool have_energy, bool z
     return MPCD_OK;
 }
 
-// a8: counting sort by cell on the counts of accumulator set `s`.
-int do_sort(mpcd_t *h, int s)
+// a8: counting sort by cell on the counts of accumulator set `s`; `shift` is the grid shift of that bin
+// (the scatter recomputes each particle's cell from its position).
+int do_sort(mpcd_t *h, int s, const double shift[3])
 {
     const int ntiles = (int)((h->Nc + kScanTile - 1) / kScanTile);
     ProfScope prof(h, MPCD_PROF_SORT);
@@ -276,13 +280,11 @@ int do_sort(mpcd_t *h, int s)
     LAUNCH_CHECK(h);
     const int src = h->pcur, dst = src ^ 1;
     if (h->opt.precision == MPCD_FP64)
-        sort_scatter<double><<<grid_for(h->N, 256), 256, 0, h->stream>>>(h->N, (const double4 *)h->pos[src], (const double4 *)h->vel[src], h->tag[src],
-                                                                     h->cell[src], h->cell_start, (double4 *)h->pos[dst], (double4 *)h->vel[dst],
-                                                                     h->tag[dst], h->cell[dst]);
+        sort_scatter<double><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<double>(h, s, s, 0, 0, shift, shift, 0.0), h->cell_start, (double4 *)h->pos[dst],
+                                                                     (double4 *)h->vel[dst], h->tag[dst]);
     else
-        sort_scatter<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(h->N, (const float4 *)h->pos[src], (const float4 *)h->vel[src], h->tag[src],
-                                                                    h->cell[src], h->cell_start, (float4 *)h->pos[dst], (float4 *)h->vel[dst],
-                                                                    h->tag[dst], h->cell[dst]);
+        sort_scatter<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<float>(h, s, s, 0, 0, shift, shift, 0.0), h->cell_start, (float4 *)h->pos[dst],
+                                                                    (float4 *)h->vel[dst], h->tag[dst]);
     LAUNCH_CHECK(h);
     h->pcur = dst;
     h->sorts += 1;
@@ -301,14 +303,28 @@ int bin_accumulate(mpcd_t *h, uint64_t t)
     int rc = zero_set(h, set, true, false);
     if (rc) return rc;
     h->zeroed[set] = false;
-    rc = pass(h, kBin | kEnergy, set, set, t, t, s, h->opt.alpha);
+    rc = pass(h, kBin | kEnergy, set, set, t, t, s, s, h->opt.alpha);
     if (rc) return rc;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = s[d];
     h->ccur = set;
     h->bin_valid = true; h->bin_step = t;
-    rc = finalize(h, set, t, 0, true, false);
+    rc = finalize(h, set, t, 0, false);
     if (rc) return rc;
     h->sums_valid = true; h->energy_valid = true;
+    return MPCD_OK;
+}
+
+// Cell index of every particle under the last bin's shift, computed on demand into h->cell (allocated on first use).
+int fill_cells(mpcd_t *h)
+{
+    if (!h->bin_valid) return fail(h, MPCD_ESTATE, "no bin yet: cell indices are undefined%s");
+    if (!h->cell) { int rc = dev_alloc_t(h, &h->cell, (size_t)h->N); if (rc) return rc; }
+    const int s = h->ccur;
+    if (h->opt.precision == MPCD_FP64)
+        cells_of_particles<double><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<double>(h, s, s, 0, 0, h->shift_used, h->shift_used, 0.0), h->cell);
+    else
+        cells_of_particles<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<float>(h, s, s, 0, 0, h->shift_used, h->shift_used, 0.0), h->cell);
+    LAUNCH_CHECK(h);
     return MPCD_OK;
 }
 
@@ -409,23 +425,22 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
     h->stream = static_cast<cudaStream_t>(o.stream);
     for (int d = 0; d < 3; ++d) { h->n[d] = n[d]; h->box[d] = box[d]; }
     h->Nc = (int64_t)n[0] * n[1] * n[2];
+    if (const char *e = std::getenv("MPCD_PREFETCH_BLOCKS")) h->prefetch_blocks = std::atoll(e);
     const size_t ns = native_size(h);
     int rc = MPCD_OK;
     for (int s = 0; s < 2 && !rc; ++s) {
         rc = dev_alloc(h, &h->pos[s], (size_t)N * 4 * ns);
         if (!rc) rc = dev_alloc(h, &h->vel[s], (size_t)N * 4 * ns);
         if (!rc) rc = dev_alloc_t(h, &h->tag[s], (size_t)N);
-        if (!rc) rc = dev_alloc_t(h, &h->cell[s], (size_t)N);
         if (!rc) rc = dev_alloc_t(h, &h->acc[s], (size_t)h->Nc * 4);
         if (!rc) rc = dev_alloc_t(h, &h->qacc[s], (size_t)h->Nc);
     }
-    for (int s = 0; s < 2 && !rc; ++s) rc = dev_alloc_t(h, &h->rec[s], (size_t)h->Nc);
+    for (int s = 0; s < 2 && !rc; ++s) rc = dev_alloc_t(h, &h->rec[s], (size_t)h->Nc * kRecDoubles);
     if (!rc) rc = dev_alloc_t(h, &h->cell_start, (size_t)h->Nc + 1);
     if (!rc) rc = dev_alloc_t(h, &h->tile_sum, (size_t)((h->Nc + kScanTile - 1) / kScanTile) + 1);
     if (!rc) rc = dev_alloc_t(h, &h->d_max_occ, 64);
     if (!rc) rc = dev_alloc_t(h, &h->d_scalars, 32);
     if (!rc && o.rule == MPCD_AT) rc = ensure_at_buffers(h);
-    if (!rc && cudaMemsetAsync(h->cell[0], 0, (size_t)N * sizeof(int32_t), h->stream) != cudaSuccess) rc = fail(h, MPCD_ECUDA, "memset failed%s");
     if (!rc && o.init_state) rc = init_state(h);
     if (rc) {
         std::memcpy(g_create_error, h->err, sizeof(g_create_error));
@@ -451,7 +466,7 @@ int mpcd_stream(mpcd_t *h)
 {
     if (!h) return MPCD_EINVAL;
     const double zero[3] = {0, 0, 0};
-    int rc = pass(h, kStream, h->ccur, h->ccur, h->step, h->step, zero, h->opt.alpha);
+    int rc = pass(h, kStream, h->ccur, h->ccur, h->step, h->step, zero, zero, h->opt.alpha);
     if (rc) return rc;
     h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
     return MPCD_OK;
@@ -470,10 +485,10 @@ int mpcd_collide_srd(mpcd_t *h, double alpha)
         return fail(h, MPCD_ESTATE, "collide_srd needs mpcd_shift_and_bin for the current step first%s");
     const int set = h->ccur;
     if (h->rec_mode != 0) {
-        int rc = finalize(h, set, h->step, 0, h->energy_valid, false);
+        int rc = finalize(h, set, h->step, 0, false);
         if (rc) return rc;
     }
-    int rc = pass(h, kSRD, set, set, h->step, h->step, h->shift_used, alpha);
+    int rc = pass(h, kSRD, set, set, h->step, h->step, h->shift_used, h->shift_used, alpha);
     if (rc) return rc;
     h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
     return MPCD_OK;
@@ -490,9 +505,9 @@ int mpcd_collide_at(mpcd_t *h)
     rc = zero_set(h, set, false, true);
     if (rc) return rc;
     h->at_zeroed[set] = false;
-    rc = pass(h, kATDraw, set, set, h->step, h->step, h->shift_used, h->opt.alpha);       // second reduction
-    if (!rc) rc = finalize(h, set, h->step, 1, h->energy_valid, false);
-    if (!rc) rc = pass(h, kATApply, set, set, h->step, h->step, h->shift_used, h->opt.alpha);
+    rc = pass(h, kATDraw, set, set, h->step, h->step, h->shift_used, h->shift_used, h->opt.alpha);       // second reduction
+    if (!rc) rc = finalize(h, set, h->step, 1, false);
+    if (!rc) rc = pass(h, kATApply, set, set, h->step, h->step, h->shift_used, h->shift_used, h->opt.alpha);
     if (rc) return rc;
     h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
     return MPCD_OK;
@@ -502,7 +517,7 @@ int mpcd_sort(mpcd_t *h)
 {
     if (!h) return MPCD_EINVAL;
     if (!(h->bin_valid && h->sums_valid)) return fail(h, MPCD_ESTATE, "sort needs a valid bin (mpcd_shift_and_bin)%s");
-    return do_sort(h, h->ccur);
+    return do_sort(h, h->ccur, h->shift_used);
 }
 
 int mpcd_step(mpcd_t *h, int32_t nsteps)
@@ -517,39 +532,40 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     if (rc) return rc;
     const double alpha = h->opt.alpha;
     uint64_t t = h->step;
-    double s[3];
-    auto shift_for = [&](uint64_t step) {
-        draw_shift(h, step, s);
-        if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) s[d] = (double)(float)s[d];
+    double s[3], sn[3];                             // grid shift of step t (being collided) and of step t + 1 (being binned)
+    auto shift_for = [&](uint64_t step, double out[3]) {
+        draw_shift(h, step, out);
+        if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) out[d] = (double)(float)out[d];   // A5
     };
     // accumulator set and record set of step k are k & 1
     // first block: stream + bin + accumulate for step t
     int set = (int)(t & 1);
     rc = zero_set(h, set, true, at);
     if (rc) return rc;
-    shift_for(t);
+    shift_for(t, s);
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
-    rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), set, set, t, t, s, alpha);
+    rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), set, set, t, t, s, s, alpha);
     if (rc) return rc;
-    if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
-    rc = finalize(h, set, t, at ? 1 : 0, energy, nsteps > 1);
+    if (sort_due(h, t)) { rc = do_sort(h, set, s); if (rc) return rc; }
+    rc = finalize(h, set, t, at ? 1 : 0, nsteps > 1);
     if (rc) return rc;
     // steady state: collide(t) fused with stream + bin + accumulate (t + 1): one pass per step
     for (int32_t j = 1; j < nsteps; ++j) {
         const int nxt = set ^ 1;
         rc = zero_set(h, nxt, true, at);            // no-op: the previous finalize zeroed it
         if (rc) return rc;
-        shift_for(t + 1);
+        shift_for(t + 1, sn);
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
-        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe, set, nxt, t, t + 1, s, alpha);
+        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe, set, nxt, t, t + 1, s, sn, alpha);
         if (rc) return rc;
         set = nxt; t += 1;
-        if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
-        rc = finalize(h, set, t, at ? 1 : 0, energy, j + 1 < nsteps);
+        for (int d = 0; d < 3; ++d) s[d] = sn[d];
+        if (sort_due(h, t)) { rc = do_sort(h, set, s); if (rc) return rc; }
+        rc = finalize(h, set, t, at ? 1 : 0, j + 1 < nsteps);
         if (rc) return rc;
     }
     // last collision
-    rc = pass(h, at ? kATApply : kSRD, set, set, t, t, s, alpha);
+    rc = pass(h, at ? kATApply : kSRD, set, set, t, t, s, s, alpha);
     if (rc) return rc;
     h->ccur = set;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = s[d];
@@ -566,7 +582,11 @@ int mpcd_get_state(mpcd_t *h, void *pos4, void *vel4, uint32_t *tag, int32_t *ce
     if (pos4) CUDA_TRY(h, cudaMemcpyAsync(pos4, h->pos[h->pcur], vb, cudaMemcpyDeviceToHost, h->stream));
     if (vel4) CUDA_TRY(h, cudaMemcpyAsync(vel4, h->vel[h->pcur], vb, cudaMemcpyDeviceToHost, h->stream));
     if (tag) CUDA_TRY(h, cudaMemcpyAsync(tag, h->tag[h->pcur], (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
-    if (cell) CUDA_TRY(h, cudaMemcpyAsync(cell, h->cell[h->pcur], (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
+    if (cell && h->bin_valid) {                       // without a bin the cell indices are unspecified: the buffer is left untouched
+        int rc = fill_cells(h);
+        if (rc) return rc;
+        CUDA_TRY(h, cudaMemcpyAsync(cell, h->cell, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
+    }
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     if (step) *step = h->step;
     return MPCD_OK;
@@ -669,7 +689,11 @@ int mpcd_device_ptrs(mpcd_t *h, void **pos4, void **vel4, uint32_t **tag, int32_
     if (pos4) *pos4 = h->pos[h->pcur];
     if (vel4) *vel4 = h->vel[h->pcur];
     if (tag) *tag = h->tag[h->pcur];
-    if (cell) *cell = h->cell[h->pcur];
+    if (cell) {
+        int rc = fill_cells(h);
+        if (rc) return rc;
+        *cell = h->cell;
+    }
     return MPCD_OK;
 }
 

@@ -12,7 +12,7 @@
 //
 // The steady-state step of mpcd_step is ONE launch with kSRD|kStream|kBin: the collision of
 // step t fused with the streaming, binning and accumulation of step t+1, so each particle's
-// 36 bytes are read once and written once per step.
+// 32 bytes (pos4 + vel4) are read once and written once per step.
 #pragma once
 #include "mpcd_device.cuh"
 
@@ -20,55 +20,78 @@ namespace mpcdk {
 
 enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u };
 
-// Per-cell record the collision gathers: 64 bytes, 64-byte aligned (never straddles a line).
-struct alignas(64) CellRec {
-    double u[3];      // mean velocity
-    double r[3];      // SRD: rotation axis.  AT: u - sum(dv)/N_c  (eq. 4 without dv_i)
-    double kT;        // cell temperature, 0 if N_c < 2 (A11)
-    long long count;  // N_c
-};
-
 template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
     typename Vec4<T>::type *vel;
     uint32_t *tag;
-    int32_t *cell;
-    const CellRec *rec;   // results of the step being collided
+    const double *rec;    // results of the step being collided: kRecDoubles per cell
     double *acc;          // accumulators of the step being binned: {Sx, Sy, Sz, N} per cell
     double *qacc;         // sum |v|^2 per cell (kEnergy)
     double *at_acc;       // {Dx, Dy, Dz, -} per cell (AT second reduction)
     int64_t N;
+    int64_t prefetch;     // particles ahead of this block whose pos/vel lines are pulled into L2 (0 = off)
     int32_t n[3];
-    T dt, L[3], shift[3], inv_a;
+    T dt, L[3], inv_a;
+    T shift[3];           // grid shift of the step being binned
     double cos_a, sin_a, sigma;
     uint64_t seed, step_collide, step_bin;
 };
 
 constexpr int kPassThreads = 256;
 
+// a3 (A6, A8): linear index of the collision cell of position p under grid shift s.
+template <typename T, typename V4>
+__device__ __forceinline__ int cell_of(const V4 &p, const T (&s)[3], T inv_a, const int32_t (&n)[3])
+{
+    const int ix = bin_axis<T>(p.x, s[0], inv_a, n[0]);
+    const int iy = bin_axis<T>(p.y, s[1], inv_a, n[1]);
+    const int iz = bin_axis<T>(p.z, s[2], inv_a, n[2]);
+    return ix + n[0] * (iy + n[1] * iz);
+}
+
+// The cell index of the last binning is cached in the fourth component of the velocity vector, as in
+// the paper ("cached into the fourth element of the particle velocity vector"): vel.w is
+// loaded and stored with the 16-byte vector anyway, so the cache costs no HBM traffic, where a separate
+// int32 array would cost 8 bytes per particle-step.  At the ABI vel.w stays unspecified padding (A9).
+__device__ __forceinline__ float cell_to_w(int c, float) { return __int_as_float(c); }
+__device__ __forceinline__ double cell_to_w(int c, double) { return __longlong_as_double((long long)c); }
+__device__ __forceinline__ int w_to_cell(float w) { return __float_as_int(w); }
+__device__ __forceinline__ int w_to_cell(double w) { return (int)__double_as_longlong(w); }
+
+#ifndef MPCD_MINBLOCKS
+#define MPCD_MINBLOCKS 1
+#endif
 template <typename T, unsigned F>
-__global__ void __launch_bounds__(kPassThreads) particle_pass(const PassArgs<T> a)
+__global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(const PassArgs<T> a)
 {
     using V4 = typename Vec4<T>::type;
-    __shared__ WarpScratch ws[(F & (kBin | kATDraw)) ? kPassThreads / 32 : 1];
+    __shared__ WarpScratch ws[(F & (kBin | kATDraw | kSRD | kATApply)) ? kPassThreads / 32 : 1];
+    WarpScratch &w = ws[(F & (kBin | kATDraw | kSRD | kATApply)) ? (threadIdx.x >> 5) : 0];
     const int64_t i = (int64_t)blockIdx.x * kPassThreads + threadIdx.x;
     const bool valid = i < a.N;
+    const int inactive = -1 - (int)(threadIdx.x & 31);
     V4 p = {}, v = {};
-    int c = 0;
     uint32_t tag = 0;
+    if (a.prefetch > 0) {        // the lines a later block will stream: 32 particles x sizeof(V4) per warp and array
+        constexpr int kLines = (int)(32 * sizeof(V4) / 128);
+        const int lane = threadIdx.x & 31;
+        const int64_t j = i - lane + a.prefetch;
+        if (lane < 2 * kLines && j + 32 <= a.N) {
+            const char *base = lane < kLines ? reinterpret_cast<const char *>(a.pos + j) : reinterpret_cast<const char *>(a.vel + j);
+            prefetch_l2(base + 128 * (lane < kLines ? lane : lane - kLines));
+        }
+    }
     if (valid) {
+        v = load4(a.vel + i);
         if (F & (kStream | kBin)) p = load4(a.pos + i);
-        if (F & (kSRD | kStream | kBin)) { if (!(F & kATApply)) v = load4(a.vel + i); }
-        if (F & (kSRD | kATApply) || ((F & kATDraw) && !(F & kBin))) c = a.cell[i];
         if (F & (kATApply | kATDraw)) tag = a.tag[i];
     }
+    int c = valid ? w_to_cell(v.w) : inactive;                   // cell of the last binning (the step being collided)
     if (F & kSRD) {
+        double2 r0, r1, r2;                                      // Alg. 1 lines 2-4: the cell's mean velocity and axis
+        warp_gather_rec(a.rec, w, c, r0, r1, r2);
         if (valid) {
-            // Alg. 1 lines 2-4: gather the cell's mean velocity and axis (3 x 16 B of one 64-B record)
-            const double *r = reinterpret_cast<const double *>(a.rec + c);
-            const f64x4 r0 = ld256_nc(r);                                    // one full sector
-            const double2 r2 = __ldg(reinterpret_cast<const double2 *>(r + 4));
-            const double ux = r0.x, uy = r0.y, uz = r0.z, nx = r0.w, ny = r2.x, nz = r2.y;
+            const double ux = r0.x, uy = r0.y, uz = r1.x, nx = r1.y, ny = r2.x, nz = r2.y;
             const double wx = (double)v.x - ux, wy = (double)v.y - uy, wz = (double)v.z - uz;   // lines 5-6
             const double ndw = nx * wx + ny * wy + nz * wz;                                    // line 7
             const double omc = 1.0 - a.cos_a;
@@ -76,18 +99,15 @@ __global__ void __launch_bounds__(kPassThreads) particle_pass(const PassArgs<T> 
             const double ry = wy * a.cos_a + (nz * wx - nx * wz) * a.sin_a + ny * ndw * omc;
             const double rz = wz * a.cos_a + (nx * wy - ny * wx) * a.sin_a + nz * ndw * omc;
             v.x = (T)(ux + rx); v.y = (T)(uy + ry); v.z = (T)(uz + rz);                          // lines 11-12
-            store4(a.vel + i, v);
         }
     }
     if (F & kATApply) {
+        double2 r0, r1, r2;                                      // r = u - D/N_c
+        warp_gather_rec(a.rec, w, c, r0, r1, r2);
         if (valid) {
             double g0, g1, g2;
             draw_gauss3(a.seed, a.step_collide, tag, g0, g1, g2);
-            const double *r = reinterpret_cast<const double *>(a.rec + c);               // r[] = u - D/N_c
-            const double2 r1 = __ldg(reinterpret_cast<const double2 *>(r + 2)), r2 = __ldg(reinterpret_cast<const double2 *>(r + 4));
             v.x = (T)(r1.y + a.sigma * g0); v.y = (T)(r2.x + a.sigma * g1); v.z = (T)(r2.y + a.sigma * g2);
-            v.w = T(0);
-            store4(a.vel + i, v);
         }
     }
     if (F & kStream) {
@@ -99,40 +119,42 @@ __global__ void __launch_bounds__(kPassThreads) particle_pass(const PassArgs<T> 
         }
     }
     if (F & kBin) {
-        int c2 = -1 - (int)(threadIdx.x & 31);
-        if (valid) {
-            const int ix = bin_axis<T>(p.x, a.shift[0], a.inv_a, a.n[0]);
-            const int iy = bin_axis<T>(p.y, a.shift[1], a.inv_a, a.n[1]);
-            const int iz = bin_axis<T>(p.z, a.shift[2], a.inv_a, a.n[2]);
-            c2 = ix + a.n[0] * (iy + a.n[1] * iz);                    // A8
-            a.cell[i] = c2;
-        }
-        warp_cell_accumulate<true, (F & kEnergy) != 0>(a.acc, a.qacc, ws[threadIdx.x >> 5], c2, (double)v.x, (double)v.y, (double)v.z);
-        c = c2;
+        c = valid ? cell_of<T>(p, a.shift, a.inv_a, a.n) : inactive;
+        v.w = cell_to_w(c, T(0));
     }
+    if ((F & (kSRD | kATApply | kBin)) && valid) store4(a.vel + i, v);
+    if (F & kBin) warp_cell_accumulate<T, true, (F & kEnergy) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
     if (F & kATDraw) {
         double g0 = 0, g1 = 0, g2 = 0;
         if (valid) draw_gauss3(a.seed, a.step_bin, tag, g0, g1, g2);
-        warp_cell_accumulate<false, false>(a.at_acc, nullptr, ws[threadIdx.x >> 5], valid ? c : -1 - (int)(threadIdx.x & 31),
-                                           a.sigma * g0, a.sigma * g1, a.sigma * g2);
+        warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, a.sigma * g0, a.sigma * g1, a.sigma * g2);
     }
 }
 
+// Cell index of every particle (the cache in vel.w) as an int32 array, on demand (mpcd_get_state, mpcd_device_ptrs).
+template <typename T>
+__global__ void __launch_bounds__(256) cells_of_particles(const PassArgs<T> a, int32_t *cell)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= a.N) return;
+    cell[i] = w_to_cell(load4(a.vel + i).w);
+}
+
 // ---------------------------------------------------------------------------------------
-// a5. Per-cell finalize: u = S / N_c, E_rel = KE - M_c u^2 / 2 (A12), kT_c (A11), the
-// random axis or, for AT, u - D / N_c; tracks the largest occupancy
-// and zeroes the OTHER accumulator set so the next step can accumulate into it.
+// a5. Per-cell finalize: u = S / N_c, the random axis or,
+// for AT, u - D / N_c; tracks the largest occupancy and zeroes the OTHER accumulator set so
+// the next step can accumulate into it.  The cell temperature (eq. 3; A11, A12)
+// is a function of the sums and is evaluated where it is consumed (cell_unpack, cell_thermo):
+// storing it per cell every step would cost HBM traffic nothing on the SRD path reads.
 // ---------------------------------------------------------------------------------------
 struct FinalizeArgs {
-    const double *acc; const double *qacc; const double *at_acc;   // this step
+    const double *acc; const double *at_acc;                       // this step
     double *acc_next; double *qacc_next; double *at_acc_next;      // zeroed for the next step (may be NULL)
-    CellRec *rec;
+    double *rec;
     int *max_occupancy;
     int64_t Nc;
-    double m;
     uint64_t seed, step;
     int at_mode;      // 0: r = axis; 1: r = u - D/N_c
-    int have_energy;
 };
 
 constexpr int kFinCells = 2;     // cells per thread: all loads are issued before any is used (memory-level parallelism)
@@ -140,21 +162,13 @@ constexpr int kFinCells = 2;     // cells per thread: all loads are issued befor
 __global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
 {
     const int64_t c0 = (int64_t)blockIdx.x * (256 * kFinCells) + threadIdx.x;
-    double2 s0[kFinCells], s1[kFinCells], d0[kFinCells], d1[kFinCells];
-    double qq[kFinCells];
-    int n[kFinCells];
+    f64x4 s[kFinCells], d[kFinCells];
 #pragma unroll
     for (int k = 0; k < kFinCells; ++k) {
         const int64_t c = c0 + 256 * k;
-        n[k] = 0;
         if (c < a.Nc) {
-            s0[k] = reinterpret_cast<const double2 *>(a.acc + 4 * c)[0];
-            s1[k] = reinterpret_cast<const double2 *>(a.acc + 4 * c)[1];
-            qq[k] = a.have_energy ? a.qacc[c] : 0.0;
-            if (a.at_mode) {
-                d0[k] = reinterpret_cast<const double2 *>(a.at_acc + 4 * c)[0];
-                d1[k] = reinterpret_cast<const double2 *>(a.at_acc + 4 * c)[1];
-            }
+            s[k] = ld256(a.acc + 4 * c);
+            if (a.at_mode) d[k] = ld256(a.at_acc + 4 * c);
         }
     }
     int nmax = 0;
@@ -162,35 +176,30 @@ __global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
     for (int k = 0; k < kFinCells; ++k) {
         const int64_t c = c0 + 256 * k;
         if (c >= a.Nc) continue;
-        const double dn = s1[k].y;
-        n[k] = (int)dn;
-        double u[3] = {0, 0, 0}, kT = 0.0;
-        if (n[k] > 0) { u[0] = s0[k].x / dn; u[1] = s0[k].y / dn; u[2] = s1[k].x / dn; }
-        if (a.have_energy && n[k] >= 2) {
-            const double erel = 0.5 * a.m * (qq[k] - dn * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
-            kT = 2.0 * erel / (3.0 * (double)(n[k] - 1));
-        }
-        double r[3] = {0, 0, 0};
+        const double dn = s[k].w;
+        const int n = (int)dn;
+        double u[3] = {0, 0, 0}, r[3] = {0, 0, 0};
+        if (n > 0) { u[0] = s[k].x / dn; u[1] = s[k].y / dn; u[2] = s[k].z / dn; }
         if (a.at_mode) {
-            if (n[k] > 0) { r[0] = u[0] - d0[k].x / dn; r[1] = u[1] - d0[k].y / dn; r[2] = u[2] - d1[k].x / dn; }
+            if (n > 0) { r[0] = u[0] - d[k].x / dn; r[1] = u[1] - d[k].y / dn; r[2] = u[2] - d[k].z / dn; }
         } else {
             draw_axis(a.seed, a.step, (uint32_t)c, r[0], r[1], r[2]);
         }
-        double2 *out = reinterpret_cast<double2 *>(a.rec + c);
-        out[0] = double2{u[0], u[1]};
-        out[1] = double2{u[2], r[0]};
-        out[2] = double2{r[1], r[2]};
-        out[3] = double2{kT, __longlong_as_double((long long)n[k])};
+        if (kRecDoubles == 8) {
+            st256(a.rec + 8 * c, u[0], u[1], u[2], r[0]);
+            st256(a.rec + 8 * c + 4, r[1], r[2], 0.0, 0.0);
+        } else {
+            double2 *out = reinterpret_cast<double2 *>(a.rec + kRecDoubles * c);
+            out[0] = double2{u[0], u[1]};
+            out[1] = double2{u[2], r[0]};
+            out[2] = double2{r[1], r[2]};
+        }
         if (a.acc_next) {
-            reinterpret_cast<double2 *>(a.acc_next + 4 * c)[0] = double2{0.0, 0.0};
-            reinterpret_cast<double2 *>(a.acc_next + 4 * c)[1] = double2{0.0, 0.0};
+            st256(a.acc_next + 4 * c, 0.0, 0.0, 0.0, 0.0);
             if (a.qacc_next) a.qacc_next[c] = 0.0;
         }
-        if (a.at_acc_next) {
-            reinterpret_cast<double2 *>(a.at_acc_next + 4 * c)[0] = double2{0.0, 0.0};
-            reinterpret_cast<double2 *>(a.at_acc_next + 4 * c)[1] = double2{0.0, 0.0};
-        }
-        nmax = n[k] > nmax ? n[k] : nmax;
+        if (a.at_acc_next) st256(a.at_acc_next + 4 * c, 0.0, 0.0, 0.0, 0.0);
+        nmax = n > nmax ? n : nmax;
     }
     const int wmax = __reduce_max_sync(0xffffffffu, nmax);
     if ((threadIdx.x & 31) == 0 && wmax > 0) atomicMax(a.max_occupancy, wmax);
@@ -230,18 +239,28 @@ __global__ void __launch_bounds__(256) cell_thermo(const double *acc, const doub
     block_sum_to_global<6>(v, out);
 }
 
-// Unpack the cell arrays for mpcd_get_cells (SoA outputs on the device, copied by the host).
-__global__ void __launch_bounds__(256) cell_unpack(const double *acc, const double *qacc, const CellRec *rec, int64_t Nc, double m,
+// Unpack the cell arrays for mpcd_get_cells (SoA outputs on the device, copied by the host); the
+// cell temperature kT_c = 2 E_rel / (3 (N_c - 1)), E_rel = KE - M_c u^2 / 2 (eq. 3; A11, A12).
+__global__ void __launch_bounds__(256) cell_unpack(const double *acc, const double *qacc, const double *rec, int64_t Nc, double m,
                                                    int32_t *count, double *sumv3, double *ke, double *u3, double *axis3, double *kTc)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
-    if (count) count[c] = (int32_t)acc[4 * c + 3];
+    const double *r = rec + kRecDoubles * c;
+    const double dn = acc[4 * c + 3];
+    if (count) count[c] = (int32_t)dn;
     if (sumv3) { sumv3[3 * c] = acc[4 * c]; sumv3[3 * c + 1] = acc[4 * c + 1]; sumv3[3 * c + 2] = acc[4 * c + 2]; }
     if (ke) ke[c] = 0.5 * m * qacc[c];
-    if (u3) { u3[3 * c] = rec[c].u[0]; u3[3 * c + 1] = rec[c].u[1]; u3[3 * c + 2] = rec[c].u[2]; }
-    if (axis3) { axis3[3 * c] = rec[c].r[0]; axis3[3 * c + 1] = rec[c].r[1]; axis3[3 * c + 2] = rec[c].r[2]; }
-    if (kTc) kTc[c] = rec[c].kT;
+    if (u3) { u3[3 * c] = r[0]; u3[3 * c + 1] = r[1]; u3[3 * c + 2] = r[2]; }
+    if (axis3) { axis3[3 * c] = r[3]; axis3[3 * c + 1] = r[4]; axis3[3 * c + 2] = r[5]; }
+    if (kTc) {
+        double kT = 0.0;
+        if (dn >= 2.0) {
+            const double erel = 0.5 * m * (qacc[c] - dn * (r[0] * r[0] + r[1] * r[1] + r[2] * r[2]));
+            kT = 2.0 * erel / (3.0 * (dn - 1.0));
+        }
+        kTc[c] = kT;
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -319,21 +338,19 @@ __global__ void __launch_bounds__(kScanThreads) scan_cells(const double *acc, in
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256) sort_scatter(int64_t N, const typename Vec4<T>::type *pos, const typename Vec4<T>::type *vel,
-                                                    const uint32_t *tag, const int32_t *cell, int32_t *cursor,
-                                                    typename Vec4<T>::type *pos2, typename Vec4<T>::type *vel2, uint32_t *tag2, int32_t *cell2)
+__global__ void __launch_bounds__(256) sort_scatter(const PassArgs<T> a /* pos, vel, tag, shift: the current bin */, int32_t *cursor,
+                                                    typename Vec4<T>::type *pos2, typename Vec4<T>::type *vel2, uint32_t *tag2)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const int c = cell[i];
-    const auto p = load4(pos + i);
-    const auto v = load4(vel + i);
-    const uint32_t t = tag[i];
+    if (i >= a.N) return;
+    const auto p = load4(a.pos + i);
+    const auto v = load4(a.vel + i);
+    const uint32_t t = a.tag[i];
+    const int c = w_to_cell(v.w);
     const int dst = atomicAdd(cursor + c, 1);
     store4(pos2 + dst, p);
     store4(vel2 + dst, v);
     tag2[dst] = t;
-    cell2[dst] = c;
 }
 
 // ---------------------------------------------------------------------------------------
