@@ -34,7 +34,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_1801_10187_b200 import synth  # noqa: E402
+from paper_1801_10187_b200 import replicas, synth  # noqa: E402
 
 METRIC = "mpcd_particle_steps_per_s"
 UNIT = "particle-steps/s"
@@ -58,12 +58,17 @@ def measured_peak():
 
 
 def ncu_traffic(workload: str, precision: str):
-    """DRAM bytes per launch of the fused kernel from the committed ncu capture, if any."""
+    """DRAM bytes per launch of the fused kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the
+    committed `ncu --set full` summary profiles/ncu_traffic.csv (workload,precision,bytes,source), if any."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f).get(f"{workload}/{precision}")
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for line in f:
+                w = [x.strip() for x in line.split(",")]
+                if len(w) >= 3 and w[0] == workload and w[1] == precision:
+                    return float(w[2])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -186,7 +191,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-particles", type=int, default=8_000_000, help="cpu_baseline sample size (particles)")
-    ap.add_argument("--cpu-steps", type=int, default=12)
+    ap.add_argument("--cpu-steps", type=int, default=40)
     ap.add_argument("--ref-particles", type=int, default=2_000_000, help="--impl reference sample size per step")
     args = ap.parse_args()
     cfg = synth.CONFIGS[args.config]
@@ -211,13 +216,12 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier(dist if world > 1 else None)
         torch.cuda.synchronize(dev)
 
     dtype = np.float32 if args.precision == "mixed" else np.float64
     n, M = cfg["n"], cfg["M"]
-    seed = cfg["seed"] + rank
+    seed = replicas.replica_seed(cfg["seed"], rank)
     pos, vel, tag = synth.solvent(n, M, seed=seed, dtype=dtype)
     N = pos.shape[0]
     sim = MPCD([float(x) for x in n], N, seed=seed, precision=args.precision, rule=cfg["rule"], sort_period=args.sort_period,
@@ -237,11 +241,7 @@ def main():
         barrier()
     ms = ev0.elapsed_time(ev1)
     launches = sim.stats()["kernel_launches"] - l0
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * N * args.steps / (ms_max * 1e-3)
+    value, ms_max = replicas.whole_job_throughput(float(N) * args.steps, ms, dist if world > 1 else None, dev)
 
     # ---- per-kernel durations, live, CUDA events on the library's stream ----
     sim.set_profiling(True)
