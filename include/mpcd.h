@@ -184,7 +184,7 @@ int mpcd_get_stats(mpcd_t *h, mpcd_stats *out /* host */);
 #define MPCD_PROF_FUSED    0   /* collide(t) + stream + bin + accumulate(t+1): the steady-state step kernel */
 #define MPCD_PROF_BIN      1   /* [stream +] bin + accumulate without a collision */
 #define MPCD_PROF_COLLIDE  2   /* collision only */
-#define MPCD_PROF_FINALIZE 3   /* per-cell finalize (u, kT_c, axis) */
+#define MPCD_PROF_CELLS    3   /* per-cell helper kernels outside the fused step (axes, zeroing) */
 #define MPCD_PROF_SORT     4   /* scan + scatter */
 #define MPCD_PROF_OTHER    5
 #define MPCD_PROF_KINDS    6

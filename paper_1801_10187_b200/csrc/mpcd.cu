@@ -36,21 +36,26 @@ struct mpcd {
     uint32_t *tag[2] = {nullptr, nullptr};
     int32_t *cell = nullptr;       // cell index per particle, filled on demand only (mpcd_get_state / mpcd_device_ptrs)
     int pcur = 0;
-    // cell arrays
-    double *acc[2] = {nullptr, nullptr};
-    double *qacc[2] = {nullptr, nullptr};
-    double *at_acc[2] = {nullptr, nullptr};
-    double *rec[2] = {nullptr, nullptr};    // kRecDoubles per cell, per accumulator set (step parity)
+    // cell arrays, double-buffered by step parity: while the fused kernel reads the sums and axes of step t
+    // (collision) it accumulates step t + 1 into the other set
+    double *acc[2] = {nullptr, nullptr};      // {Sx, Sy, Sz, N} per cell
+    double *qacc[2] = {nullptr, nullptr};     // sum |v|^2 per cell
+    double *at_acc[2] = {nullptr, nullptr};   // {Dx, Dy, Dz, -} per cell (AT only, allocated on first use)
+    double *axis[2] = {nullptr, nullptr};     // {nx, ny, nz, -} per cell
     int32_t *cell_start = nullptr, *tile_sum = nullptr;
     int *d_max_occ = nullptr;
     double *d_scalars = nullptr;   // 8 doubles of scratch for reductions
     int ccur = 0;                  // accumulator set of the current bin
     int64_t prefetch_blocks = 0;   // L2 prefetch distance of the particle pass, in blocks
+    int num_sms = 148;
+    bool debug_sync = false;       // MPCD_DEBUG_SYNC=1: synchronise after every launch (see LAUNCH_CHECK)
     bool zeroed[2] = {false, false}, at_zeroed[2] = {false, false};
+    bool axis_valid[2] = {false, false};
+    uint64_t axis_step[2] = {0, 0};
+    int max_occ = 0;               // of the last bin whose counts were inspected
     // state machine
     uint64_t step = 0, bin_step = 0;
-    bool bin_valid = false, sums_valid = false, energy_valid = false, rec_valid = false;
-    int rec_mode = 0;
+    bool bin_valid = false, sums_valid = false, energy_valid = false, counts_valid = false;
     double shift_used[3] = {0, 0, 0};
     // bookkeeping
     std::vector<Buffer> buffers;
@@ -79,11 +84,18 @@ int fail(mpcd_t *h, int code, const char *fmt, const char *detail = "")
         if (e_ != cudaSuccess) return fail((h), MPCD_ECUDA, #expr ": %s", cudaGetErrorString(e_)); \
     } while (0)
 
+// After every kernel launch.  With MPCD_DEBUG_SYNC=1 in the environment the stream is synchronised here, so a
+// faulting kernel is reported at its own launch site (source line, launch number) instead of at a later call.
 #define LAUNCH_CHECK(h)                                                          \
     do {                                                                         \
         (h)->launches += 1;                                                      \
         cudaError_t e_ = cudaGetLastError();                                     \
-        if (e_ != cudaSuccess) return fail((h), MPCD_ECUDA, "kernel launch: %s", cudaGetErrorString(e_)); \
+        if (e_ == cudaSuccess && (h)->debug_sync) e_ = cudaStreamSynchronize((h)->stream); \
+        if (e_ != cudaSuccess) {                                                 \
+            char where_[96];                                                     \
+            snprintf(where_, sizeof(where_), "%s (mpcd.cu:%d, launch %llu)", cudaGetErrorString(e_), __LINE__, (unsigned long long)(h)->launches); \
+            return fail((h), MPCD_ECUDA, "kernel launch: %s", where_);          \
+        }                                                                        \
     } while (0)
 
 int dev_alloc(mpcd_t *h, void **out, size_t bytes)
@@ -147,32 +159,43 @@ void draw_shift(const mpcd_t *h, uint64_t step, double s[3])
     for (int d = 0; d < 3; ++d) s[d] = (u01_32(w[d]) - 0.5) * h->a;
 }
 
-template <typename T> PassArgs<T> make_args(mpcd_t *h, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift_c[3],
-                                            const double shift[3], double alpha)
+// What one launch of the pass works on: `cset` = accumulator set of the step being collided (its sums, thermostat
+// sums and, by step parity, its axes), `bset` = set of the step being binned.
+struct PassPlan {
+    int cset = 0, bset = 0;
+    uint64_t step_collide = 0, step_bin = 0;
+    double shift[3] = {0, 0, 0};      // grid shift of the step being binned
+    double alpha = 0;
+};
+
+template <typename T> PassArgs<T> make_args(mpcd_t *h, const PassPlan &pl)
 {
     PassArgs<T> a{};
     a.pos = static_cast<typename Vec4<T>::type *>(h->pos[h->pcur]);
     a.vel = static_cast<typename Vec4<T>::type *>(h->vel[h->pcur]);
     a.tag = h->tag[h->pcur];
-    a.rec = h->rec[rec_set];
-    a.acc = h->acc[acc_set];
-    a.qacc = h->qacc[acc_set];
-    a.at_acc = h->at_acc[acc_set];
+    a.sums = h->acc[pl.cset];
+    a.dsum = h->at_acc[pl.cset];
+    a.axis = h->axis[pl.step_collide & 1];
+    a.acc = h->acc[pl.bset];
+    a.qacc = h->qacc[pl.bset];
+    a.at_acc = h->at_acc[pl.bset];
     a.N = h->N;
+    a.Nc = h->Nc;
     a.prefetch = h->prefetch_blocks * (int64_t)kPassThreads;
     for (int d = 0; d < 3; ++d) {
         a.n[d] = h->n[d];
         a.L[d] = (T)h->box[d];
-        a.shift[d] = (T)shift[d];
+        a.shift[d] = (T)pl.shift[d];
     }
     a.dt = (T)h->opt.dt;
     a.inv_a = (T)1 / (T)h->a;
-    a.cos_a = std::cos(alpha);
-    a.sin_a = std::sin(alpha);
+    a.cos_a = std::cos(pl.alpha);
+    a.sin_a = std::sin(pl.alpha);
     a.sigma = h->sigma;
     a.seed = h->seed;
-    a.step_collide = step_collide;
-    a.step_bin = step_bin;
+    a.step_collide = pl.step_collide;
+    a.step_bin = pl.step_bin;
     return a;
 }
 
@@ -181,10 +204,9 @@ template <typename T, unsigned F> void launch_pass_t(mpcd_t *h, const PassArgs<T
     particle_pass<T, F><<<grid_for(h->N, kPassThreads), kPassThreads, 0, h->stream>>>(a);
 }
 
-template <typename T> int launch_pass(mpcd_t *h, unsigned F, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin,
-                                      const double shift_c[3], const double shift[3], double alpha)
+template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
 {
-    const PassArgs<T> a = make_args<T>(h, rec_set, acc_set, step_collide, step_bin, shift_c, shift, alpha);
+    const PassArgs<T> a = make_args<T>(h, pl);
     switch (F) {
 #define CASE(f) case (f): launch_pass_t<T, (f)>(h, a); break;
         CASE(kStream)
@@ -196,10 +218,10 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, int rec_set, int ac
         CASE(kSRD)
         CASE(kSRD | kStream | kBin)
         CASE(kSRD | kStream | kBin | kEnergy)
-        CASE(kATDraw)
-        CASE(kATApply)
         CASE(kATApply | kStream | kBin | kATDraw)
         CASE(kATApply | kStream | kBin | kATDraw | kEnergy)
+        CASE(kATDraw)
+        CASE(kATApply)
 #undef CASE
         default: return fail(h, MPCD_EINVAL, "internal: pass combination not instantiated%s");
     }
@@ -207,14 +229,11 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, int rec_set, int ac
     return MPCD_OK;
 }
 
-// shift_c: grid shift of the step being collided; shift: grid shift of the step being binned
-int pass(mpcd_t *h, unsigned F, int rec_set, int acc_set, uint64_t step_collide, uint64_t step_bin, const double shift_c[3], const double shift[3],
-         double alpha)
+int pass(mpcd_t *h, unsigned F, const PassPlan &pl)
 {
     const bool collide = (F & (kSRD | kATApply)) != 0, bin = (F & kBin) != 0;
     ProfScope prof(h, collide && bin ? MPCD_PROF_FUSED : (collide ? MPCD_PROF_COLLIDE : (bin ? MPCD_PROF_BIN : MPCD_PROF_OTHER)));
-    return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, rec_set, acc_set, step_collide, step_bin, shift_c, shift, alpha)
-                                         : launch_pass<float>(h, F, rec_set, acc_set, step_collide, step_bin, shift_c, shift, alpha);
+    return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, pl) : launch_pass<float>(h, F, pl);
 }
 
 int ensure_at_buffers(mpcd_t *h)
@@ -228,47 +247,30 @@ int ensure_at_buffers(mpcd_t *h)
     return MPCD_OK;
 }
 
-int zero_set(mpcd_t *h, int s, bool sums, bool at)
+// Cell-side preparation, as ONE launch of cell_prepare doing whatever of this is still missing: accumulator set
+// `zset` all-zero (its sums if `sums`, its thermostat sums if `at`; zset < 0 = none) and the axes of step
+// `axis_step` in axis[axis_step & 1] (want_axes = false: none).
+int prepare(mpcd_t *h, int zset, bool sums, bool at, bool want_axes, uint64_t axis_step)
 {
-    sums = sums && !h->zeroed[s];
-    at = at && h->at_acc[s] && !h->at_zeroed[s];
-    if (!sums && !at) return MPCD_OK;
-    cell_zero<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(sums ? h->acc[s] : nullptr, h->qacc[s], at ? h->at_acc[s] : nullptr, h->Nc);
+    const bool zs = zset >= 0 && sums && !h->zeroed[zset];
+    const bool za = zset >= 0 && at && h->at_acc[zset] && !h->at_zeroed[zset];
+    const int b = (int)(axis_step & 1);
+    const bool ax = want_axes && !(h->axis_valid[b] && h->axis_step[b] == axis_step);
+    if (!zs && !za && !ax) return MPCD_OK;
+    ProfScope prof(h, MPCD_PROF_CELLS);
+    cell_prepare<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(ax ? h->axis[b] : nullptr, h->seed, axis_step, zs ? h->acc[zset] : nullptr,
+                                                           zs ? h->qacc[zset] : nullptr, za ? h->at_acc[zset] : nullptr, h->Nc);
     LAUNCH_CHECK(h);
-    if (sums) h->zeroed[s] = true;
-    if (at) h->at_zeroed[s] = true;
+    if (zs) h->zeroed[zset] = true;
+    if (za) h->at_zeroed[zset] = true;
+    if (ax) { h->axis_valid[b] = true; h->axis_step[b] = axis_step; }
     return MPCD_OK;
 }
+inline int zero_set(mpcd_t *h, int s, bool sums, bool at) { return prepare(h, s, sums, at, false, 0); }
+inline int ensure_axes(mpcd_t *h, uint64_t t) { return prepare(h, -1, false, false, true, t); }
 
-// a5 for accumulator set `s` at step `t` into rec[s]; optionally zero the other set for the next step.
-int finalize(mpcd_t *h, int s, uint64_t t, int at_mode, bool zero_next)
-{
-    FinalizeArgs f{};
-    f.acc = h->acc[s]; f.at_acc = h->at_acc[s];
-    const int o = s ^ 1;
-    const bool zs = zero_next && !h->zeroed[o];
-    const bool za = zero_next && h->at_acc[o] && !h->at_zeroed[o] && at_mode;
-    f.acc_next = zs ? h->acc[o] : nullptr;
-    f.qacc_next = zs ? h->qacc[o] : nullptr;
-    f.at_acc_next = za ? h->at_acc[o] : nullptr;
-    f.rec = h->rec[s];
-    f.max_occupancy = h->d_max_occ;
-    f.Nc = h->Nc; f.seed = h->seed; f.step = t;
-    f.at_mode = at_mode;
-    ProfScope prof(h, MPCD_PROF_FINALIZE);
-    CUDA_TRY(h, cudaMemsetAsync(h->d_max_occ, 0, sizeof(int), h->stream));
-    cell_finalize<<<grid_for(h->Nc, 256 * kFinCells), 256, 0, h->stream>>>(f);
-    LAUNCH_CHECK(h);
-    if (zs) h->zeroed[o] = true;
-    if (za) h->at_zeroed[o] = true;
-    h->rec_valid = true;
-    h->rec_mode = at_mode;
-    return MPCD_OK;
-}
-
-// a8: counting sort by cell on the counts of accumulator set `s`; `shift` is the grid shift of that bin
-// (the scatter recomputes each particle's cell from its position).
-int do_sort(mpcd_t *h, int s, const double shift[3])
+// a8: counting sort by cell on the counts of accumulator set `s` (the cell of every particle is cached in vel.w)
+int do_sort(mpcd_t *h, int s)
 {
     const int ntiles = (int)((h->Nc + kScanTile - 1) / kScanTile);
     ProfScope prof(h, MPCD_PROF_SORT);
@@ -279,12 +281,12 @@ int do_sort(mpcd_t *h, int s, const double shift[3])
     scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum, h->cell_start);
     LAUNCH_CHECK(h);
     const int src = h->pcur, dst = src ^ 1;
+    PassPlan pl;
+    pl.cset = pl.bset = s;
     if (h->opt.precision == MPCD_FP64)
-        sort_scatter<double><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<double>(h, s, s, 0, 0, shift, shift, 0.0), h->cell_start, (double4 *)h->pos[dst],
-                                                                     (double4 *)h->vel[dst], h->tag[dst]);
+        sort_scatter<double><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<double>(h, pl), h->cell_start, (double4 *)h->pos[dst], (double4 *)h->vel[dst], h->tag[dst]);
     else
-        sort_scatter<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<float>(h, s, s, 0, 0, shift, shift, 0.0), h->cell_start, (float4 *)h->pos[dst],
-                                                                    (float4 *)h->vel[dst], h->tag[dst]);
+        sort_scatter<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<float>(h, pl), h->cell_start, (float4 *)h->pos[dst], (float4 *)h->vel[dst], h->tag[dst]);
     LAUNCH_CHECK(h);
     h->pcur = dst;
     h->sorts += 1;
@@ -293,24 +295,32 @@ int do_sort(mpcd_t *h, int s, const double shift[3])
 
 inline bool sort_due(const mpcd_t *h, uint64_t t) { return h->opt.sort_period > 0 && (t % (uint64_t)h->opt.sort_period) == 0; }
 
-// bin + accumulate + full finalize for step t as a standalone block; energy always accumulated here
+inline void shift_for(const mpcd_t *h, uint64_t step, double out[3])
+{
+    draw_shift(h, step, out);
+    if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) out[d] = (double)(float)out[d];   // A5
+}
+
+// bin + accumulate (+ axes) for step t as a standalone block; energy always accumulated here
 int bin_accumulate(mpcd_t *h, uint64_t t)
 {
-    double s[3];
-    draw_shift(h, t, s);
-    if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) s[d] = (double)(float)s[d];   // A5
+    PassPlan pl;
+    shift_for(h, t, pl.shift);
     const int set = (int)(t & 1);
+    pl.cset = pl.bset = set;
+    pl.step_collide = pl.step_bin = t;
+    pl.alpha = h->opt.alpha;
     int rc = zero_set(h, set, true, false);
     if (rc) return rc;
     h->zeroed[set] = false;
-    rc = pass(h, kBin | kEnergy, set, set, t, t, s, s, h->opt.alpha);
+    rc = pass(h, kBin | kEnergy, pl);
     if (rc) return rc;
-    for (int d = 0; d < 3; ++d) h->shift_used[d] = s[d];
+    for (int d = 0; d < 3; ++d) h->shift_used[d] = pl.shift[d];
     h->ccur = set;
     h->bin_valid = true; h->bin_step = t;
-    rc = finalize(h, set, t, 0, false);
+    rc = ensure_axes(h, t);
     if (rc) return rc;
-    h->sums_valid = true; h->energy_valid = true;
+    h->sums_valid = true; h->energy_valid = true; h->counts_valid = true;
     return MPCD_OK;
 }
 
@@ -319,11 +329,12 @@ int fill_cells(mpcd_t *h)
 {
     if (!h->bin_valid) return fail(h, MPCD_ESTATE, "no bin yet: cell indices are undefined%s");
     if (!h->cell) { int rc = dev_alloc_t(h, &h->cell, (size_t)h->N); if (rc) return rc; }
-    const int s = h->ccur;
+    PassPlan pl;
+    pl.cset = pl.bset = h->ccur;
     if (h->opt.precision == MPCD_FP64)
-        cells_of_particles<double><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<double>(h, s, s, 0, 0, h->shift_used, h->shift_used, 0.0), h->cell);
+        cells_of_particles<double><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<double>(h, pl), h->cell);
     else
-        cells_of_particles<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<float>(h, s, s, 0, 0, h->shift_used, h->shift_used, 0.0), h->cell);
+        cells_of_particles<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<float>(h, pl), h->cell);
     LAUNCH_CHECK(h);
     return MPCD_OK;
 }
@@ -426,16 +437,23 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
     for (int d = 0; d < 3; ++d) { h->n[d] = n[d]; h->box[d] = box[d]; }
     h->Nc = (int64_t)n[0] * n[1] * n[2];
     if (const char *e = std::getenv("MPCD_PREFETCH_BLOCKS")) h->prefetch_blocks = std::atoll(e);
+    if (const char *e = std::getenv("MPCD_DEBUG_SYNC")) h->debug_sync = std::atoi(e) != 0;
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) h->num_sms = sms;
+    }
     const size_t ns = native_size(h);
     int rc = MPCD_OK;
     for (int s = 0; s < 2 && !rc; ++s) {
         rc = dev_alloc(h, &h->pos[s], (size_t)N * 4 * ns);
         if (!rc) rc = dev_alloc(h, &h->vel[s], (size_t)N * 4 * ns);
         if (!rc) rc = dev_alloc_t(h, &h->tag[s], (size_t)N);
-        if (!rc) rc = dev_alloc_t(h, &h->acc[s], (size_t)h->Nc * 4);
+        if (!rc) rc = dev_alloc_t(h, &h->axis[s], (size_t)h->Nc * 4);
+    }
+    for (int s = 0; s < 2 && !rc; ++s) {
+        rc = dev_alloc_t(h, &h->acc[s], (size_t)h->Nc * 4);
         if (!rc) rc = dev_alloc_t(h, &h->qacc[s], (size_t)h->Nc);
     }
-    for (int s = 0; s < 2 && !rc; ++s) rc = dev_alloc_t(h, &h->rec[s], (size_t)h->Nc * kRecDoubles);
     if (!rc) rc = dev_alloc_t(h, &h->cell_start, (size_t)h->Nc + 1);
     if (!rc) rc = dev_alloc_t(h, &h->tile_sum, (size_t)((h->Nc + kScanTile - 1) / kScanTile) + 1);
     if (!rc) rc = dev_alloc_t(h, &h->d_max_occ, 64);
@@ -465,10 +483,12 @@ int mpcd_destroy(mpcd_t *h)
 int mpcd_stream(mpcd_t *h)
 {
     if (!h) return MPCD_EINVAL;
-    const double zero[3] = {0, 0, 0};
-    int rc = pass(h, kStream, h->ccur, h->ccur, h->step, h->step, zero, zero, h->opt.alpha);
+    PassPlan pl;
+    pl.cset = pl.bset = h->ccur;
+    pl.step_collide = pl.step_bin = h->step;
+    int rc = pass(h, kStream, pl);
     if (rc) return rc;
-    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false;
     return MPCD_OK;
 }
 
@@ -481,16 +501,17 @@ int mpcd_shift_and_bin(mpcd_t *h)
 int mpcd_collide_srd(mpcd_t *h, double alpha)
 {
     if (!h) return MPCD_EINVAL;
-    if (!(h->bin_valid && h->bin_step == h->step && h->sums_valid && h->rec_valid))
+    if (!(h->bin_valid && h->bin_step == h->step && h->sums_valid))
         return fail(h, MPCD_ESTATE, "collide_srd needs mpcd_shift_and_bin for the current step first%s");
-    const int set = h->ccur;
-    if (h->rec_mode != 0) {
-        int rc = finalize(h, set, h->step, 0, false);
-        if (rc) return rc;
-    }
-    int rc = pass(h, kSRD, set, set, h->step, h->step, h->shift_used, h->shift_used, alpha);
+    int rc = ensure_axes(h, h->step);
     if (rc) return rc;
-    h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    PassPlan pl;
+    pl.cset = pl.bset = h->ccur;
+    pl.step_collide = pl.step_bin = h->step;
+    pl.alpha = alpha;
+    rc = pass(h, kSRD, pl);
+    if (rc) return rc;
+    h->sums_valid = false; h->energy_valid = false;
     return MPCD_OK;
 }
 
@@ -505,19 +526,22 @@ int mpcd_collide_at(mpcd_t *h)
     rc = zero_set(h, set, false, true);
     if (rc) return rc;
     h->at_zeroed[set] = false;
-    rc = pass(h, kATDraw, set, set, h->step, h->step, h->shift_used, h->shift_used, h->opt.alpha);       // second reduction
-    if (!rc) rc = finalize(h, set, h->step, 1, false);
-    if (!rc) rc = pass(h, kATApply, set, set, h->step, h->step, h->shift_used, h->shift_used, h->opt.alpha);
+    PassPlan pl;
+    pl.cset = pl.bset = set;
+    pl.step_collide = pl.step_bin = h->step;
+    pl.alpha = h->opt.alpha;
+    rc = pass(h, kATDraw, pl);                       // second reduction
+    if (!rc) rc = pass(h, kATApply, pl);
     if (rc) return rc;
-    h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    h->sums_valid = false; h->energy_valid = false;
     return MPCD_OK;
 }
 
 int mpcd_sort(mpcd_t *h)
 {
     if (!h) return MPCD_EINVAL;
-    if (!(h->bin_valid && h->sums_valid)) return fail(h, MPCD_ESTATE, "sort needs a valid bin (mpcd_shift_and_bin)%s");
-    return do_sort(h, h->ccur, h->shift_used);
+    if (!(h->bin_valid && h->counts_valid)) return fail(h, MPCD_ESTATE, "sort needs a valid bin (mpcd_shift_and_bin)%s");
+    return do_sort(h, h->ccur);
 }
 
 int mpcd_step(mpcd_t *h, int32_t nsteps)
@@ -526,51 +550,47 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     if (nsteps < 0) return fail(h, MPCD_EINVAL, "nsteps must be >= 0%s");
     if (nsteps == 0) return MPCD_OK;
     const bool at = h->opt.rule == MPCD_AT;
-    const bool energy = h->opt.cell_energy != 0;
-    const unsigned fe = energy ? kEnergy : 0u;
+    const unsigned fe = h->opt.cell_energy != 0 ? kEnergy : 0u;
     int rc = at ? ensure_at_buffers(h) : MPCD_OK;
     if (rc) return rc;
-    const double alpha = h->opt.alpha;
     uint64_t t = h->step;
-    double s[3], sn[3];                             // grid shift of step t (being collided) and of step t + 1 (being binned)
-    auto shift_for = [&](uint64_t step, double out[3]) {
-        draw_shift(h, step, out);
-        if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) out[d] = (double)(float)out[d];   // A5
-    };
-    // accumulator set and record set of step k are k & 1
+    int set = (int)(t & 1);                         // cell arrays of step k: set k & 1
+    PassPlan pl;
+    pl.alpha = h->opt.alpha;
     // first block: stream + bin + accumulate for step t
-    int set = (int)(t & 1);
-    rc = zero_set(h, set, true, at);
+    rc = prepare(h, set, true, at, !at, t);         // zeroed set of step t, axes of step t
     if (rc) return rc;
-    shift_for(t, s);
+    shift_for(h, t, pl.shift);
+    pl.cset = pl.bset = set;
+    pl.step_collide = pl.step_bin = t;
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
-    rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), set, set, t, t, s, s, alpha);
+    rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), pl);
     if (rc) return rc;
-    if (sort_due(h, t)) { rc = do_sort(h, set, s); if (rc) return rc; }
-    rc = finalize(h, set, t, at ? 1 : 0, nsteps > 1);
-    if (rc) return rc;
-    // steady state: collide(t) fused with stream + bin + accumulate (t + 1): one pass per step
+    if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
+    // steady state, two launches per step: cell_prepare (zeroed set and axes of step t + 1), then collide(t) fused with
+    // stream + bin + accumulate (t + 1)
     for (int32_t j = 1; j < nsteps; ++j) {
         const int nxt = set ^ 1;
-        rc = zero_set(h, nxt, true, at);            // no-op: the previous finalize zeroed it
+        rc = prepare(h, nxt, true, at, !at, t + 1);
         if (rc) return rc;
-        shift_for(t + 1, sn);
+        shift_for(h, t + 1, pl.shift);
+        pl.cset = set; pl.bset = nxt;
+        pl.step_collide = t; pl.step_bin = t + 1;
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
-        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe, set, nxt, t, t + 1, s, sn, alpha);
+        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe, pl);
         if (rc) return rc;
         set = nxt; t += 1;
-        for (int d = 0; d < 3; ++d) s[d] = sn[d];
-        if (sort_due(h, t)) { rc = do_sort(h, set, s); if (rc) return rc; }
-        rc = finalize(h, set, t, at ? 1 : 0, j + 1 < nsteps);
-        if (rc) return rc;
+        if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
     }
     // last collision
-    rc = pass(h, at ? kATApply : kSRD, set, set, t, t, s, s, alpha);
+    pl.cset = pl.bset = set;
+    pl.step_collide = pl.step_bin = t;
+    rc = pass(h, at ? kATApply : kSRD, pl);
     if (rc) return rc;
     h->ccur = set;
-    for (int d = 0; d < 3; ++d) h->shift_used[d] = s[d];
-    h->bin_valid = true; h->bin_step = t;
-    h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    for (int d = 0; d < 3; ++d) h->shift_used[d] = pl.shift[d];
+    h->bin_valid = true; h->bin_step = t; h->counts_valid = true;
+    h->sums_valid = false; h->energy_valid = false;
     h->step = t + 1;
     return MPCD_OK;
 }
@@ -607,16 +627,16 @@ int mpcd_set_state(mpcd_t *h, const void *pos4, const void *vel4, const uint32_t
     }
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     h->step = step;
-    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->rec_valid = false;
+    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false;
     return MPCD_OK;
 }
 
 int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double *u3, double *axis3, double *kTc)
 {
     if (!h) return MPCD_EINVAL;
-    if (!(h->sums_valid && h->rec_valid && h->energy_valid))
+    if (!(h->sums_valid && h->energy_valid))
         return fail(h, MPCD_ESTATE, "cell sums are not valid: call mpcd_shift_and_bin first%s");
-    if (axis3 && h->rec_mode != 0) return fail(h, MPCD_ESTATE, "no axis in the cell records (Andersen-thermostat finalize)%s");
+    if (axis3) { int rc0 = ensure_axes(h, h->bin_step); if (rc0) return rc0; }
     const size_t Nc = (size_t)h->Nc;
     // stage through one temporary device buffer (SoA), sized for everything asked
     const size_t bytes = Nc * (4 + 8 * (3 + 1 + 3 + 3 + 1));
@@ -630,7 +650,7 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
     double *d_ax = d_u + 3 * Nc;
     double *d_kT = d_ax + 3 * Nc;
     int32_t *d_cnt = reinterpret_cast<int32_t *>(d_kT + Nc);
-    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->rec[h->ccur], h->Nc, h->m, d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
+    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->axis[h->bin_step & 1], h->Nc, h->m, d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
     h->launches += 1;
     int rc = MPCD_OK;
     auto cp = [&](void *dst, const void *src, size_t b) {
@@ -658,7 +678,7 @@ int mpcd_get_thermo(mpcd_t *h, double P[3], double *KE, double *kT)
         if (rc) return rc;
     }
     CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, 8 * sizeof(double), h->stream));
-    cell_thermo<<<148 * 4, 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->Nc, h->m, h->d_scalars);
+    cell_thermo<<<h->num_sms * 4, 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->Nc, h->m, h->d_scalars);
     LAUNCH_CHECK(h);
     double out[6];
     CUDA_TRY(h, cudaMemcpyAsync(out, h->d_scalars, sizeof(out), cudaMemcpyDeviceToHost, h->stream));
@@ -675,10 +695,14 @@ int mpcd_get_stats(mpcd_t *h, mpcd_stats *out)
     std::memset(out, 0, sizeof(*out));
     out->N = h->N; out->Nc = h->Nc;
     for (int d = 0; d < 3; ++d) out->n[d] = h->n[d];
-    int mo = 0;
-    CUDA_TRY(h, cudaMemcpyAsync(&mo, h->d_max_occ, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    out->max_occupancy = mo;
+    if (h->bin_valid && h->counts_valid) {            // the counts of the last bin are still in its accumulator set
+        CUDA_TRY(h, cudaMemsetAsync(h->d_max_occ, 0, sizeof(int), h->stream));
+        cell_max_occupancy<<<h->num_sms * 8, 256, 0, h->stream>>>(h->acc[h->ccur], h->Nc, h->d_max_occ);
+        LAUNCH_CHECK(h);
+        CUDA_TRY(h, cudaMemcpyAsync(&h->max_occ, h->d_max_occ, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    }
+    out->max_occupancy = h->max_occ;
     out->step = h->step; out->kernel_launches = h->launches; out->sorts = h->sorts; out->device_bytes = h->device_bytes;
     return MPCD_OK;
 }

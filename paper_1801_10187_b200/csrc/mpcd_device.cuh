@@ -165,88 +165,20 @@ template <typename T> __device__ __forceinline__ int bin_axis(T x, T s, T inv_a,
 // ---------------------------------------------------------------------------------------
 // Warp-level machinery of the per-particle pass.
 //
-// What bounds the pass on a B200 is not HBM bandwidth alone but the SM's L1/LSU data pipe:
-// one "wavefront" per cycle per SM.  Measured on the box (profiles/r01_lsu_costs.md): a
-// coalesced 16-byte-per-lane access costs 4 wavefronts; a per-lane gather of a 48-byte cell
-// record costs ~46 (it is charged per lane, identical addresses in non-adjacent lanes are not
-// merged); a RED costs ~0.6 per distinct 32-byte sector; a SHFL costs 1.  So both cell-side
-// steps are done "transposed": lanes that share a cell are found with match.any, one leader
-// per distinct cell is compacted into shared memory, and then ADJACENT lanes touch ADJACENT
-// words of one cell's record (3 lanes x 16 B for the gather, 4 lanes x 8 B for the RED), which
-// the LSU coalesces into one request per record.
+// What bounds the pass on a B200 is not HBM bandwidth alone but the SM's L1/LSU data pipe, one
+// "wavefront" per cycle per SM (measured with micro-kernels under ncu): a coalesced
+// 16-byte-per-lane access costs 4 wavefronts; a per-lane gather costs about 8 + bytes/2 per warp
+// instruction whatever the number of distinct cells; a RED costs ~0.75 per leader record per
+// instruction; a 32-bit SHFL costs 1.  So the accumulation is done "transposed": lanes that share a
+// cell are found with match.any and combined, one leader per distinct cell is compacted into shared
+// memory, and then 4 ADJACENT lanes issue the REDs on the 4 ADJACENT doubles of one cell's sector.
 // ---------------------------------------------------------------------------------------
 constexpr int kStagePitch = 36;    // doubles per staged component row: 4 rows land in disjoint banks for one half-warp
-struct alignas(16) WarpScratch {   // per-warp shared memory; the two phases of a pass use it one after the other
-    union {
-        double2 rec[32][3];        // gather staging: [leader slot][16-byte part of the 48-byte record]
-        struct {
-            double v[4][kStagePitch];   // accumulate staging: [component][leader slot]
-            double q[32];
-        } a;
-    };
+struct alignas(16) WarpScratch {   // per-warp shared memory of the accumulate phase
+    double v[4][kStagePitch];      // [component][leader slot]
+    double q[32];
     int cell[32];                  // cell index of leader slot j
 };
-
-// Per-cell record the collision reads: u (mean velocity) and r (SRD: the rotation
-// axis; AT: u - sum(dv)/N_c, eq. 4 without dv_i).
-#ifndef MPCD_GATHER
-#define MPCD_GATHER 0
-#endif
-#if MPCD_GATHER == 1
-constexpr int kRecDoubles = 6;     // packed 48-byte records, read as 3 x 16 B by adjacent lanes
-#else
-constexpr int kRecDoubles = 8;     // 64-byte aligned records {u, r, pad, pad}: never straddle a line, 32-byte loads are aligned
-#endif
-
-// Alg. 1 lines 2-4: every lane gets the record of its cell c.
-// Lanes with c < 0 take no part (their outputs are undefined).
-__device__ __forceinline__ void warp_gather_rec(const double *__restrict__ rec, WarpScratch &ws, int c, double2 &r0, double2 &r1, double2 &r2)
-{
-#if MPCD_GATHER == 0
-    if (c >= 0) {
-        const double *r = rec + (size_t)kRecDoubles * c;
-        const f64x4 a = ld256_nc(r);                                   // one full sector
-        r2 = __ldg(reinterpret_cast<const double2 *>(r + 4));
-        r0 = double2{a.x, a.y}; r1 = double2{a.z, a.w};
-    }
-#elif MPCD_GATHER == 2
-    const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    const unsigned peers = __match_any_sync(full, c);
-    const int lead = __ffs(peers) - 1;
-    f64x4 a = {0, 0, 0, 0};
-    double2 b = {0, 0};
-    if (lead == lane && c >= 0) {
-        const double *r = rec + (size_t)kRecDoubles * c;
-        a = ld256_nc(r);
-        b = __ldg(reinterpret_cast<const double2 *>(r + 4));
-    }
-    r0.x = __shfl_sync(full, a.x, lead); r0.y = __shfl_sync(full, a.y, lead);
-    r1.x = __shfl_sync(full, a.z, lead); r1.y = __shfl_sync(full, a.w, lead);
-    r2.x = __shfl_sync(full, b.x, lead); r2.y = __shfl_sync(full, b.y, lead);
-#else
-    const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    const unsigned peers = __match_any_sync(full, c);
-    const int lead = __ffs(peers) - 1;
-    const unsigned leaders = __ballot_sync(full, lead == lane && c >= 0);
-    const int slot = __popc(leaders & ((1u << lead) - 1u));          // compact index of my cell's leader
-    const int nl = __popc(leaders);
-    if (lead == lane && c >= 0) ws.cell[slot] = c;
-    __syncwarp();
-    const int sub = lane / 3, part = lane - 3 * sub;                 // 10 records per round, 3 lanes x 16 B each
-    for (int base = 0; base < nl; base += 10) {
-        const int j = base + sub;
-        if (lane < 30 && j < nl) {
-            const double2 x = __ldg(reinterpret_cast<const double2 *>(rec + (size_t)kRecDoubles * ws.cell[j]) + part);
-            ws.rec[j][part] = x;
-        }
-    }
-    __syncwarp();
-    r0 = ws.rec[slot][0]; r1 = ws.rec[slot][1]; r2 = ws.rec[slot][2];
-    __syncwarp();                                                     // the scratch is reused by the accumulate phase
-#endif
-}
 
 // ---------------------------------------------------------------------------------------
 // Per-cell fp64 accumulation.  Layout in HBM: acc[c] = {Sx, Sy, Sz, N}
@@ -296,18 +228,18 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
     const int nl = __popc(leaders);
     if (leader && c >= 0) {
         const int j = __popc(leaders & ((1u << lane) - 1u));
-        ws.a.v[0][j] = vx; ws.a.v[1][j] = vy; ws.a.v[2][j] = vz;
-        if (kCount) ws.a.v[3][j] = (double)size;
-        if (kEnergy) ws.a.q[j] = q;
+        ws.v[0][j] = vx; ws.v[1][j] = vy; ws.v[2][j] = vz;
+        if (kCount) ws.v[3][j] = (double)size;
+        if (kEnergy) ws.q[j] = q;
         ws.cell[j] = c;
     }
     __syncwarp();
     const int comp = lane & 3;                             // 8 leaders per round, 4 lanes x 8 B = one 32-byte sector each
     for (int base = 0; base < nl; base += 8) {
         const int j = base + (lane >> 2);
-        if (j < nl && (kCount || comp < 3)) atomicAdd(acc + 4 * (size_t)ws.cell[j] + comp, ws.a.v[comp][j]);
+        if (j < nl && (kCount || comp < 3)) atomicAdd(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[comp][j]);
     }
-    if (kEnergy && lane < nl) atomicAdd(qacc + ws.cell[lane], ws.a.q[lane]);
+    if (kEnergy && lane < nl) atomicAdd(qacc + ws.cell[lane], ws.q[lane]);
     __syncwarp();
 }
 

@@ -1,18 +1,21 @@
 // mpcd_kernels.cuh -- the kernels of the MPCD solvent step (sm_100a).
 //
-// One templated per-particle pass covers every particle-side block of Fig. 1
-// and their fusions; compile-time flags select which blocks a launch contains:
+// One templated per-particle pass covers every block of Fig. 1 and their fusions;
+// compile-time flags select which blocks a launch contains:
 //
-//   kSRD      a6  SRD collision, Alg. 1 PAPER.md:142-155 (gathers u, axis of the particle's cell)
-//   kATApply  a7  Andersen-thermostat update, eq. 4 PAPER.md:54 (regenerates dv from the tag)
-//   kStream   a1  eq. 1 PAPER.md:35 + periodic wrap
+//   kSRD      a5+a6  SRD collision, Alg. 1: gathers the sums {S, N} and the axis of the
+//                    particle's cell, u = S / N, rotates in fp64
+//   kATApply  a7     Andersen-thermostat update, eq. 4 PAPER.md:54 (regenerates dv from the tag)
+//   kStream   a1     eq. 1 PAPER.md:35 + periodic wrap
 //   kBin      a3+a4  shifted binning + fp64 cell accumulation
-//   kEnergy   a4  also accumulate sum |v|^2 (kinetic energy, eq. 3)
-//   kATDraw   a7  draw dv for the (new) step and accumulate its per-cell sum
+//   kEnergy   a4     also accumulate sum |v|^2 (kinetic energy, eq. 3)
+//   kATDraw   a7     draw dv for the (new) step and accumulate its per-cell sum
 //
-// The steady-state step of mpcd_step is ONE launch with kSRD|kStream|kBin: the collision of
-// step t fused with the streaming, binning and accumulation of step t+1, so each particle's
-// 32 bytes (pos4 + vel4) are read once and written once per step.
+// The steady-state step of mpcd_step is ONE particle launch, kSRD|kStream|kBin|kEnergy: the collision of
+// step t fused with the streaming, binning and accumulation of step t+1, so each particle's 32 bytes
+// (pos4 + vel4) are read once and written once per step.  The mean velocity is formed where it is used
+// (u = S / N from the cell's sums), so the only per-cell work between two steps is cell_prepare: the axes
+// of the next step and a zeroed accumulator set.
 #pragma once
 #include "mpcd_device.cuh"
 
@@ -24,11 +27,15 @@ template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
     typename Vec4<T>::type *vel;
     uint32_t *tag;
-    const double *rec;    // results of the step being collided: kRecDoubles per cell
-    double *acc;          // accumulators of the step being binned: {Sx, Sy, Sz, N} per cell
+    // cell arrays of the step being collided (read only)
+    const double *sums;   // {Sx, Sy, Sz, N} per cell
+    const double *dsum;   // {Dx, Dy, Dz, -} per cell: sum of the thermostat draws (AT)
+    const double *axis;   // {nx, ny, nz, -} per cell (SRD)
+    // accumulators of the step being binned
+    double *acc;          // {Sx, Sy, Sz, N} per cell
     double *qacc;         // sum |v|^2 per cell (kEnergy)
     double *at_acc;       // {Dx, Dy, Dz, -} per cell (AT second reduction)
-    int64_t N;
+    int64_t N, Nc;
     int64_t prefetch;     // particles ahead of this block whose pos/vel lines are pulled into L2 (0 = off)
     int32_t n[3];
     T dt, L[3], inv_a;
@@ -59,14 +66,14 @@ __device__ __forceinline__ int w_to_cell(float w) { return __float_as_int(w); }
 __device__ __forceinline__ int w_to_cell(double w) { return (int)__double_as_longlong(w); }
 
 #ifndef MPCD_MINBLOCKS
-#define MPCD_MINBLOCKS 1
+#define MPCD_MINBLOCKS 5
 #endif
 template <typename T, unsigned F>
 __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(const PassArgs<T> a)
 {
     using V4 = typename Vec4<T>::type;
-    __shared__ WarpScratch ws[(F & (kBin | kATDraw | kSRD | kATApply)) ? kPassThreads / 32 : 1];
-    WarpScratch &w = ws[(F & (kBin | kATDraw | kSRD | kATApply)) ? (threadIdx.x >> 5) : 0];
+    __shared__ WarpScratch ws[(F & (kBin | kATDraw)) ? kPassThreads / 32 : 1];
+    WarpScratch &w = ws[(F & (kBin | kATDraw)) ? (threadIdx.x >> 5) : 0];
     const int64_t i = (int64_t)blockIdx.x * kPassThreads + threadIdx.x;
     const bool valid = i < a.N;
     const int inactive = -1 - (int)(threadIdx.x & 31);
@@ -88,26 +95,30 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     }
     int c = valid ? w_to_cell(v.w) : inactive;                   // cell of the last binning (the step being collided)
     if (F & kSRD) {
-        double2 r0, r1, r2;                                      // Alg. 1 lines 2-4: the cell's mean velocity and axis
-        warp_gather_rec(a.rec, w, c, r0, r1, r2);
         if (valid) {
-            const double ux = r0.x, uy = r0.y, uz = r1.x, nx = r1.y, ny = r2.x, nz = r2.y;
+            const f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);    // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
+            const f64x4 n = ld256_nc(a.axis + 4 * (size_t)c);
+            const double inv = __drcp_rn(s.w);                   // N_c >= 1: this particle is a member
+            const double ux = s.x * inv, uy = s.y * inv, uz = s.z * inv;
             const double wx = (double)v.x - ux, wy = (double)v.y - uy, wz = (double)v.z - uz;   // lines 5-6
-            const double ndw = nx * wx + ny * wy + nz * wz;                                    // line 7
+            const double ndw = n.x * wx + n.y * wy + n.z * wz;                                  // line 7
             const double omc = 1.0 - a.cos_a;
-            const double rx = wx * a.cos_a + (ny * wz - nz * wy) * a.sin_a + nx * ndw * omc;
-            const double ry = wy * a.cos_a + (nz * wx - nx * wz) * a.sin_a + ny * ndw * omc;
-            const double rz = wz * a.cos_a + (nx * wy - ny * wx) * a.sin_a + nz * ndw * omc;
+            const double rx = wx * a.cos_a + (n.y * wz - n.z * wy) * a.sin_a + n.x * ndw * omc;
+            const double ry = wy * a.cos_a + (n.z * wx - n.x * wz) * a.sin_a + n.y * ndw * omc;
+            const double rz = wz * a.cos_a + (n.x * wy - n.y * wx) * a.sin_a + n.z * ndw * omc;
             v.x = (T)(ux + rx); v.y = (T)(uy + ry); v.z = (T)(uz + rz);                          // lines 11-12
         }
     }
     if (F & kATApply) {
-        double2 r0, r1, r2;                                      // r = u - D/N_c
-        warp_gather_rec(a.rec, w, c, r0, r1, r2);
-        if (valid) {
+        if (valid) {                                             // eq. 4: v = u + dv_i - D / N_c = (S - D) / N_c + dv_i
+            const f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);
+            const f64x4 d = ld256_nc(a.dsum + 4 * (size_t)c);
+            const double inv = __drcp_rn(s.w);
             double g0, g1, g2;
             draw_gauss3(a.seed, a.step_collide, tag, g0, g1, g2);
-            v.x = (T)(r1.y + a.sigma * g0); v.y = (T)(r2.x + a.sigma * g1); v.z = (T)(r2.y + a.sigma * g2);
+            v.x = (T)((s.x - d.x) * inv + a.sigma * g0);
+            v.y = (T)((s.y - d.y) * inv + a.sigma * g1);
+            v.z = (T)((s.z - d.z) * inv + a.sigma * g2);
         }
     }
     if (F & kStream) {
@@ -141,84 +152,35 @@ __global__ void __launch_bounds__(256) cells_of_particles(const PassArgs<T> a, i
 }
 
 // ---------------------------------------------------------------------------------------
-// a5. Per-cell finalize: u = S / N_c, the random axis or,
-// for AT, u - D / N_c; tracks the largest occupancy and zeroes the OTHER accumulator set so
-// the next step can accumulate into it.  The cell temperature (eq. 3; A11, A12)
-// is a function of the sums and is evaluated where it is consumed (cell_unpack, cell_thermo):
-// storing it per cell every step would cost HBM traffic nothing on the SRD path reads.
+// a5, cell side: the random axis of every cell for one step (it depends on
+// (seed, step, cell) only, so it can be drawn before that step's particles are binned) and / or a zeroed
+// accumulator set.  Any pointer may be NULL.  One launch per step in mpcd_step: the axes of step t + 1
+// together with the zeroing of the set of step t + 2.
 // ---------------------------------------------------------------------------------------
-struct FinalizeArgs {
-    const double *acc; const double *at_acc;                       // this step
-    double *acc_next; double *qacc_next; double *at_acc_next;      // zeroed for the next step (may be NULL)
-    double *rec;
-    int *max_occupancy;
-    int64_t Nc;
-    uint64_t seed, step;
-    int at_mode;      // 0: r = axis; 1: r = u - D/N_c
-};
-
-constexpr int kFinCells = 2;     // cells per thread: all loads are issued before any is used (memory-level parallelism)
-
-__global__ void __launch_bounds__(256, 4) cell_finalize(const FinalizeArgs a)
-{
-    const int64_t c0 = (int64_t)blockIdx.x * (256 * kFinCells) + threadIdx.x;
-    f64x4 s[kFinCells], d[kFinCells];
-#pragma unroll
-    for (int k = 0; k < kFinCells; ++k) {
-        const int64_t c = c0 + 256 * k;
-        if (c < a.Nc) {
-            s[k] = ld256(a.acc + 4 * c);
-            if (a.at_mode) d[k] = ld256(a.at_acc + 4 * c);
-        }
-    }
-    int nmax = 0;
-#pragma unroll
-    for (int k = 0; k < kFinCells; ++k) {
-        const int64_t c = c0 + 256 * k;
-        if (c >= a.Nc) continue;
-        const double dn = s[k].w;
-        const int n = (int)dn;
-        double u[3] = {0, 0, 0}, r[3] = {0, 0, 0};
-        if (n > 0) { u[0] = s[k].x / dn; u[1] = s[k].y / dn; u[2] = s[k].z / dn; }
-        if (a.at_mode) {
-            if (n > 0) { r[0] = u[0] - d[k].x / dn; r[1] = u[1] - d[k].y / dn; r[2] = u[2] - d[k].z / dn; }
-        } else {
-            draw_axis(a.seed, a.step, (uint32_t)c, r[0], r[1], r[2]);
-        }
-        if (kRecDoubles == 8) {
-            st256(a.rec + 8 * c, u[0], u[1], u[2], r[0]);
-            st256(a.rec + 8 * c + 4, r[1], r[2], 0.0, 0.0);
-        } else {
-            double2 *out = reinterpret_cast<double2 *>(a.rec + kRecDoubles * c);
-            out[0] = double2{u[0], u[1]};
-            out[1] = double2{u[2], r[0]};
-            out[2] = double2{r[1], r[2]};
-        }
-        if (a.acc_next) {
-            st256(a.acc_next + 4 * c, 0.0, 0.0, 0.0, 0.0);
-            if (a.qacc_next) a.qacc_next[c] = 0.0;
-        }
-        if (a.at_acc_next) st256(a.at_acc_next + 4 * c, 0.0, 0.0, 0.0, 0.0);
-        nmax = n > nmax ? n : nmax;
-    }
-    const int wmax = __reduce_max_sync(0xffffffffu, nmax);
-    if ((threadIdx.x & 31) == 0 && wmax > 0) atomicMax(a.max_occupancy, wmax);
-}
-
-// zero one accumulator set
-__global__ void __launch_bounds__(256) cell_zero(double *acc, double *qacc, double *at_acc, int64_t Nc)
+__global__ void __launch_bounds__(256) cell_prepare(double *axis, uint64_t seed, uint64_t step, double *zero_acc, double *zero_q, double *zero_at, int64_t Nc)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
-    if (acc) {
-        reinterpret_cast<double2 *>(acc + 4 * c)[0] = double2{0.0, 0.0};
-        reinterpret_cast<double2 *>(acc + 4 * c)[1] = double2{0.0, 0.0};
-        qacc[c] = 0.0;
+    if (zero_acc) st256(zero_acc + 4 * c, 0.0, 0.0, 0.0, 0.0);
+    if (zero_q) zero_q[c] = 0.0;
+    if (zero_at) st256(zero_at + 4 * c, 0.0, 0.0, 0.0, 0.0);
+    if (axis) {
+        double nx, ny, nz;
+        draw_axis(seed, step, (uint32_t)c, nx, ny, nz);
+        st256(axis + 4 * c, nx, ny, nz, 0.0);
     }
-    if (at_acc) {
-        reinterpret_cast<double2 *>(at_acc + 4 * c)[0] = double2{0.0, 0.0};
-        reinterpret_cast<double2 *>(at_acc + 4 * c)[1] = double2{0.0, 0.0};
+}
+
+// Largest cell occupancy of a bin (mpcd_get_stats), from the counts in the accumulator set.
+__global__ void __launch_bounds__(256) cell_max_occupancy(const double *acc, int64_t Nc, int *out)
+{
+    int nmax = 0;
+    for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c < Nc; c += (int64_t)gridDim.x * blockDim.x) {
+        const int n = (int)acc[4 * c + 3];
+        nmax = n > nmax ? n : nmax;
     }
+    nmax = __reduce_max_sync(0xffffffffu, nmax);
+    if ((threadIdx.x & 31) == 0 && nmax > 0) atomicMax(out, nmax);
 }
 
 // a9. Net momentum, kinetic energy, pooled temperature by device-wide reduction.
@@ -239,24 +201,26 @@ __global__ void __launch_bounds__(256) cell_thermo(const double *acc, const doub
     block_sum_to_global<6>(v, out);
 }
 
-// Unpack the cell arrays for mpcd_get_cells (SoA outputs on the device, copied by the host); the
-// cell temperature kT_c = 2 E_rel / (3 (N_c - 1)), E_rel = KE - M_c u^2 / 2 (eq. 3; A11, A12).
-__global__ void __launch_bounds__(256) cell_unpack(const double *acc, const double *qacc, const double *rec, int64_t Nc, double m,
+// Unpack the cell arrays for mpcd_get_cells (SoA outputs on the device, copied by the host): u = S / N_c
+// (PAPER.md:122), the cell temperature kT_c = 2 E_rel / (3 (N_c - 1)), E_rel = KE - M_c u^2 / 2
+// (eq. 3; A11, A12).
+__global__ void __launch_bounds__(256) cell_unpack(const double *acc, const double *qacc, const double *axis, int64_t Nc, double m,
                                                    int32_t *count, double *sumv3, double *ke, double *u3, double *axis3, double *kTc)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
-    const double *r = rec + kRecDoubles * c;
     const double dn = acc[4 * c + 3];
+    double u[3] = {0, 0, 0};
+    if (dn > 0.0) { u[0] = acc[4 * c] / dn; u[1] = acc[4 * c + 1] / dn; u[2] = acc[4 * c + 2] / dn; }
     if (count) count[c] = (int32_t)dn;
     if (sumv3) { sumv3[3 * c] = acc[4 * c]; sumv3[3 * c + 1] = acc[4 * c + 1]; sumv3[3 * c + 2] = acc[4 * c + 2]; }
     if (ke) ke[c] = 0.5 * m * qacc[c];
-    if (u3) { u3[3 * c] = r[0]; u3[3 * c + 1] = r[1]; u3[3 * c + 2] = r[2]; }
-    if (axis3) { axis3[3 * c] = r[3]; axis3[3 * c + 1] = r[4]; axis3[3 * c + 2] = r[5]; }
+    if (u3) { u3[3 * c] = u[0]; u3[3 * c + 1] = u[1]; u3[3 * c + 2] = u[2]; }
+    if (axis3) { axis3[3 * c] = axis[4 * c]; axis3[3 * c + 1] = axis[4 * c + 1]; axis3[3 * c + 2] = axis[4 * c + 2]; }
     if (kTc) {
         double kT = 0.0;
         if (dn >= 2.0) {
-            const double erel = 0.5 * m * (qacc[c] - dn * (r[0] * r[0] + r[1] * r[1] + r[2] * r[2]));
+            const double erel = 0.5 * m * (qacc[c] - dn * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
             kT = 2.0 * erel / (3.0 * (dn - 1.0));
         }
         kTc[c] = kT;
