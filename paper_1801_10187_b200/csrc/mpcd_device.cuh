@@ -190,6 +190,11 @@ struct alignas(16) WarpScratch {   // per-warp shared memory of the accumulate p
 // the receiver, as PAPER.md:124 asks ("all reductions are performed with double-precision
 // values even if the particle velocities are stored in single precision").
 // ---------------------------------------------------------------------------------------
+#ifndef MPCD_TREE_ROUNDS
+#define MPCD_TREE_ROUNDS 0
+#endif
+constexpr int kTreeRounds = MPCD_TREE_ROUNDS;   // rounds of the in-warp combining tree before the REDs; 0 = until one lane per cell is left
+
 template <typename T, bool kCount, bool kEnergy>
 __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, double *__restrict__ qacc, WarpScratch &ws,
                                                      int c /* < 0 = inactive lane, unique per lane */, T fx, T fy, T fz)
@@ -200,36 +205,48 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
     double q = kEnergy ? (vx * vx + vy * vy + vz * vz) : 0.0;
     unsigned peers = __match_any_sync(full, c);
     const int size = __popc(peers);
-    const bool leader = (__ffs(peers) - 1) == lane;
-    int rank = __popc(peers & ((1u << lane) - 1u));
+    const int rank0 = __popc(peers & ((1u << lane) - 1u));
+    int rank = rank0, rounds = 0;
+    bool alive = true;                                     // not yet folded into a lower-ranked peer
     peers &= (0xfffffffeu << lane);                        // peers above this lane
-    if (__any_sync(full, peers != 0u)) {                   // round 1: raw particle values, native precision
+    if (kTreeRounds == 1 || __any_sync(full, peers != 0u)) {   // round 1: raw particle values, native precision
         const int next = __ffs(peers);                     // 1-based lane of the next peer, 0 = none
         const int src = next ? next - 1 : lane;
         const T tx = __shfl_sync(full, fx, src), ty = __shfl_sync(full, fy, src), tz = __shfl_sync(full, fz, src);
-        if (next) {
+        alive = !(rank & 1);
+        if (next && alive) {
             const double dx = (double)tx, dy = (double)ty, dz = (double)tz;
             vx += dx; vy += dy; vz += dz;
             if (kEnergy) q += dx * dx + dy * dy + dz * dz;
         }
-        peers &= __ballot_sync(full, !(rank & 1));         // odd-ranked lanes have been absorbed
-        rank >>= 1;
+        rounds = 1;
+        if (kTreeRounds != 1) {
+            peers &= __ballot_sync(full, alive);           // odd-ranked lanes have been absorbed
+            rank >>= 1;
+        }
     }
-    while (__any_sync(full, peers != 0u)) {                // log2(largest group) rounds in all
-        const int next = __ffs(peers);
-        const int src = next ? next - 1 : lane;
-        const double tx = __shfl_sync(full, vx, src), ty = __shfl_sync(full, vy, src), tz = __shfl_sync(full, vz, src);
-        const double tq = kEnergy ? __shfl_sync(full, q, src) : 0.0;
-        if (next) { vx += tx; vy += ty; vz += tz; q += tq; }
-        peers &= __ballot_sync(full, !(rank & 1));
-        rank >>= 1;
+    if (kTreeRounds != 1) {
+        while ((kTreeRounds == 0 || rounds < kTreeRounds) && __any_sync(full, alive && peers != 0u)) {   // log2(largest group) rounds at most
+            const int next = __ffs(peers);
+            const int src = next ? next - 1 : lane;
+            const double tx = __shfl_sync(full, vx, src), ty = __shfl_sync(full, vy, src), tz = __shfl_sync(full, vz, src);
+            const double tq = kEnergy ? __shfl_sync(full, q, src) : 0.0;
+            if (next && alive && !(rank & 1)) { vx += tx; vy += ty; vz += tz; q += tq; }
+            alive = alive && !(rank & 1);
+            peers &= __ballot_sync(full, alive);
+            rank >>= 1;
+            rounds += 1;
+        }
     }
-    const unsigned leaders = __ballot_sync(full, leader && c >= 0);
+    // a surviving lane holds the sum over the original ranks [rank0, rank0 + 2^rounds) of its group
+    const int span = 1 << rounds;
+    const int mine = size - rank0 < span ? size - rank0 : span;
+    const unsigned leaders = __ballot_sync(full, alive && c >= 0);
     const int nl = __popc(leaders);
-    if (leader && c >= 0) {
+    if (alive && c >= 0) {
         const int j = __popc(leaders & ((1u << lane) - 1u));
         ws.v[0][j] = vx; ws.v[1][j] = vy; ws.v[2][j] = vz;
-        if (kCount) ws.v[3][j] = (double)size;
+        if (kCount) ws.v[3][j] = (double)mine;
         if (kEnergy) ws.q[j] = q;
         ws.cell[j] = c;
     }

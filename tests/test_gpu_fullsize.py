@@ -166,17 +166,21 @@ def test_config2_thousand_steps_momentum_drift_and_temperature():
     g = MPCD([float(x) for x in cfg["n"]], N, seed=cfg["seed"], sort_period=25, init_state=False)
     g.set_state(pos, vel, tag)
     P0, KE0, kT0 = g.get_thermo()
-    drift, kTs = 0.0, [kT0]
+    drift, kTs, KEs = 0.0, [kT0], [KE0]
     for _ in range(20):
         g.step(50)
         P, KE, kT = g.get_thermo()
         drift = max(drift, float(np.max(np.abs(np.asarray(P) - np.asarray(P0)))) / N)   # / (N m sigma), m = sigma = 1 (A25)
-        kTs.append(kT)
+        kTs.append(kT); KEs.append(KE)
     assert g.stats()["step"] == 1000 and g.stats()["sorts"] == 40
     assert drift <= 1e-6, drift
-    # SRD conserves energy: the pooled temperature stays at its initial value up to fp32 store rounding
-    assert max(abs(k - kT0) for k in kTs) <= 2e-4, kTs
-    assert abs(kT0 - 1.0) <= 5 * np.sqrt(2.0 / (3.0 * N))      # initial draw: statistical error of kT
+    # SRD conserves energy: the total kinetic energy moves only by fp32 store rounding
+    assert max(abs(k - KE0) for k in KEs) / KE0 <= 2e-5, KEs
+    # temperature within statistical error: the pooled estimator (A11) measures KE relative to the cell means of
+    # one particular binning, whose share (~1/M of KE) fluctuates by sqrt(2 / (3 N_c)) from bin to bin: sigma ~ 2e-4
+    sigma_bin = np.sqrt(2.0 / (3.0 * 64 ** 3)) / cfg["M"]
+    assert max(abs(k - kT0) for k in kTs) <= 6 * sigma_bin, (kTs, sigma_bin)
+    assert abs(kT0 - 1.0) <= 5 * np.sqrt(2.0 / (3.0 * N))      # the initial draw itself
     s = g.get_state()
     assert np.array_equal(np.sort(s["tag"]), tag)               # no particle lost or duplicated by 40 sorts
     assert np.all((s["pos"][:, :3] >= 0) & (s["pos"][:, :3] < 64.0))
