@@ -185,9 +185,10 @@ int mpcd_get_stats(mpcd_t *h, mpcd_stats *out /* host */);
 #define MPCD_PROF_BIN      1   /* [stream +] bin + accumulate without a collision */
 #define MPCD_PROF_COLLIDE  2   /* collision only */
 #define MPCD_PROF_CELLS    3   /* per-cell helper kernels outside the fused step (axes, zeroing) */
-#define MPCD_PROF_SORT     4   /* scan + scatter */
+#define MPCD_PROF_SORT     4   /* scan of the cell counts; the scatter pass when the sort is not fused into a step kernel */
 #define MPCD_PROF_OTHER    5
-#define MPCD_PROF_KINDS    6
+#define MPCD_PROF_FUSED_SORT 6 /* the fused step kernel on a sort step: it also writes the particles out in cell order */
+#define MPCD_PROF_KINDS    7
 int mpcd_set_profiling(mpcd_t *h, int32_t on);
 int mpcd_get_profile(mpcd_t *h, double ms[MPCD_PROF_KINDS], uint64_t count[MPCD_PROF_KINDS]);
 

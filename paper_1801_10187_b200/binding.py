@@ -52,7 +52,7 @@ EXPORTS = [
     "mpcd_get_cells", "mpcd_get_shift", "mpcd_get_thermo", "mpcd_get_stats", "mpcd_device_ptrs", "mpcd_last_error",
     "mpcd_abi_version", "mpcd_build_info", "mpcd_test_philox", "mpcd_set_profiling", "mpcd_get_profile",
 ]
-PROF_KINDS = ("fused", "bin", "collide", "cells", "sort", "other")
+PROF_KINDS = ("fused", "bin", "collide", "cells", "sort", "other", "fused_sort")
 
 _lib = None
 

@@ -166,6 +166,7 @@ struct PassPlan {
     uint64_t step_collide = 0, step_bin = 0;
     double shift[3] = {0, 0, 0};      // grid shift of the step being binned
     double alpha = 0;
+    bool sort_out = false;            // kSortOut: write the particles to the duplicate arrays in cell order
 };
 
 template <typename T> PassArgs<T> make_args(mpcd_t *h, const PassPlan &pl)
@@ -180,6 +181,10 @@ template <typename T> PassArgs<T> make_args(mpcd_t *h, const PassPlan &pl)
     a.acc = h->acc[pl.bset];
     a.qacc = h->qacc[pl.bset];
     a.at_acc = h->at_acc[pl.bset];
+    a.pos_out = static_cast<typename Vec4<T>::type *>(h->pos[h->pcur ^ 1]);
+    a.vel_out = static_cast<typename Vec4<T>::type *>(h->vel[h->pcur ^ 1]);
+    a.tag_out = h->tag[h->pcur ^ 1];
+    a.cursor = h->cell_start;
     a.N = h->N;
     a.Nc = h->Nc;
     a.prefetch = h->prefetch_blocks * (int64_t)kPassThreads;
@@ -220,6 +225,10 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
         CASE(kSRD | kStream | kBin | kEnergy)
         CASE(kATApply | kStream | kBin | kATDraw)
         CASE(kATApply | kStream | kBin | kATDraw | kEnergy)
+        CASE(kSRD | kStream | kBin | kSortOut)
+        CASE(kSRD | kStream | kBin | kEnergy | kSortOut)
+        CASE(kATApply | kStream | kBin | kATDraw | kSortOut)
+        CASE(kATApply | kStream | kBin | kATDraw | kEnergy | kSortOut)
         CASE(kATDraw)
         CASE(kATApply)
 #undef CASE
@@ -232,7 +241,7 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
 int pass(mpcd_t *h, unsigned F, const PassPlan &pl)
 {
     const bool collide = (F & (kSRD | kATApply)) != 0, bin = (F & kBin) != 0;
-    ProfScope prof(h, collide && bin ? MPCD_PROF_FUSED : (collide ? MPCD_PROF_COLLIDE : (bin ? MPCD_PROF_BIN : MPCD_PROF_OTHER)));
+    ProfScope prof(h, collide && bin ? ((F & kSortOut) ? MPCD_PROF_FUSED_SORT : MPCD_PROF_FUSED) : (collide ? MPCD_PROF_COLLIDE : (bin ? MPCD_PROF_BIN : MPCD_PROF_OTHER)));
     return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, pl) : launch_pass<float>(h, F, pl);
 }
 
@@ -269,8 +278,8 @@ int prepare(mpcd_t *h, int zset, bool sums, bool at, bool want_axes, uint64_t ax
 inline int zero_set(mpcd_t *h, int s, bool sums, bool at) { return prepare(h, s, sums, at, false, 0); }
 inline int ensure_axes(mpcd_t *h, uint64_t t) { return prepare(h, -1, false, false, true, t); }
 
-// a8: counting sort by cell on the counts of accumulator set `s` (the cell of every particle is cached in vel.w)
-int do_sort(mpcd_t *h, int s)
+// a8, first half: exclusive scan of the per-cell counts of accumulator set `s` -> cell_start (the write cursors)
+int scan_counts(mpcd_t *h, int s)
 {
     const int ntiles = (int)((h->Nc + kScanTile - 1) / kScanTile);
     ProfScope prof(h, MPCD_PROF_SORT);
@@ -280,6 +289,16 @@ int do_sort(mpcd_t *h, int s)
     LAUNCH_CHECK(h);
     scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum, h->cell_start);
     LAUNCH_CHECK(h);
+    return MPCD_OK;
+}
+
+// a8 as a pass of its own: counting sort by cell on the counts of accumulator set `s` (the cell of every particle is
+// cached in vel.w).  Inside mpcd_step the scatter is done by the next fused kernel instead (kSortOut).
+int do_sort(mpcd_t *h, int s)
+{
+    int rc = scan_counts(h, s);
+    if (rc) return rc;
+    ProfScope prof(h, MPCD_PROF_SORT);
     const int src = h->pcur, dst = src ^ 1;
     PassPlan pl;
     pl.cset = pl.bset = s;
@@ -566,22 +585,25 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
     rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), pl);
     if (rc) return rc;
-    if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
+    bool sort_pending = sort_due(h, t);            // sort by the cells of step t: done by the next fused kernel on its way out
     // steady state, two launches per step: cell_prepare (zeroed set and axes of step t + 1), then collide(t) fused with
     // stream + bin + accumulate (t + 1)
     for (int32_t j = 1; j < nsteps; ++j) {
         const int nxt = set ^ 1;
         rc = prepare(h, nxt, true, at, !at, t + 1);
         if (rc) return rc;
+        if (sort_pending) { rc = scan_counts(h, set); if (rc) return rc; }
         shift_for(h, t + 1, pl.shift);
         pl.cset = set; pl.bset = nxt;
         pl.step_collide = t; pl.step_bin = t + 1;
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
-        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe, pl);
+        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
         if (rc) return rc;
+        if (sort_pending) { h->pcur ^= 1; h->sorts += 1; }
         set = nxt; t += 1;
-        if (sort_due(h, t)) { rc = do_sort(h, set); if (rc) return rc; }
+        sort_pending = sort_due(h, t);
     }
+    if (sort_pending) { rc = do_sort(h, set); if (rc) return rc; }
     // last collision
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;

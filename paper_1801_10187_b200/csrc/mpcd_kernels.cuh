@@ -10,6 +10,9 @@
 //   kBin      a3+a4  shifted binning + fp64 cell accumulation
 //   kEnergy   a4     also accumulate sum |v|^2 (kinetic energy, eq. 3)
 //   kATDraw   a7     draw dv for the (new) step and accumulate its per-cell sum
+//   kSortOut  a8     sort by cell on the way out: instead of in place, the particle is written
+//                    to slot cell_start[c] + (atomic cursor) of the duplicate arrays, c = its cell in the step
+//                    being collided; the separate read-and-scatter pass of the sort disappears
 //
 // The steady-state step of mpcd_step is ONE particle launch, kSRD|kStream|kBin|kEnergy: the collision of
 // step t fused with the streaming, binning and accumulation of step t+1, so each particle's 32 bytes
@@ -21,7 +24,7 @@
 
 namespace mpcdk {
 
-enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u };
+enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u };
 
 template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
@@ -35,6 +38,11 @@ template <typename T> struct PassArgs {
     double *acc;          // {Sx, Sy, Sz, N} per cell
     double *qacc;         // sum |v|^2 per cell (kEnergy)
     double *at_acc;       // {Dx, Dy, Dz, -} per cell (AT second reduction)
+    // kSortOut: the duplicate particle arrays and the per-cell write cursor (exclusive scan of the counts)
+    typename Vec4<T>::type *pos_out;
+    typename Vec4<T>::type *vel_out;
+    uint32_t *tag_out;
+    int32_t *cursor;
     int64_t N, Nc;
     int64_t prefetch;     // particles ahead of this block whose pos/vel lines are pulled into L2 (0 = off)
     int32_t n[3];
@@ -91,9 +99,11 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     if (valid) {
         v = load4(a.vel + i);
         if (F & (kStream | kBin)) p = load4(a.pos + i);
-        if (F & (kATApply | kATDraw)) tag = a.tag[i];
+        if (F & (kATApply | kATDraw | kSortOut)) tag = a.tag[i];
     }
     int c = valid ? w_to_cell(v.w) : inactive;                   // cell of the last binning (the step being collided)
+    int64_t o = i;                                               // where this particle is written
+    if ((F & kSortOut) && valid) o = atomicAdd(a.cursor + c, 1); // issued early: its latency hides behind the gather
     if (F & kSRD) {
         if (valid) {
             const f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);    // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
@@ -126,14 +136,15 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
             p.x = stream_wrap<T>(p.x, v.x, a.dt, a.L[0]);
             p.y = stream_wrap<T>(p.y, v.y, a.dt, a.L[1]);
             p.z = stream_wrap<T>(p.z, v.z, a.dt, a.L[2]);
-            store4(a.pos + i, p);
+            store4(((F & kSortOut) ? a.pos_out : a.pos) + o, p);
         }
     }
     if (F & kBin) {
         c = valid ? cell_of<T>(p, a.shift, a.inv_a, a.n) : inactive;
         v.w = cell_to_w(c, T(0));
     }
-    if ((F & (kSRD | kATApply | kBin)) && valid) store4(a.vel + i, v);
+    if ((F & (kSRD | kATApply | kBin)) && valid) store4(((F & kSortOut) ? a.vel_out : a.vel) + o, v);
+    if ((F & kSortOut) && valid) a.tag_out[o] = tag;
     if (F & kBin) warp_cell_accumulate<T, true, (F & kEnergy) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
     if (F & kATDraw) {
         double g0 = 0, g1 = 0, g2 = 0;
