@@ -52,7 +52,10 @@ template <typename T> struct PassArgs {
     uint64_t seed, step_collide, step_bin;
 };
 
-constexpr int kPassThreads = 256;
+#ifndef MPCD_PASS_THREADS
+#define MPCD_PASS_THREADS 256
+#endif
+constexpr int kPassThreads = MPCD_PASS_THREADS;
 
 // a3 (A6, A8): linear index of the collision cell of position p under grid shift s.
 template <typename T, typename V4>
