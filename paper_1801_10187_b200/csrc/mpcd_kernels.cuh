@@ -53,7 +53,7 @@ template <typename T> struct PassArgs {
 };
 
 #ifndef MPCD_PASS_THREADS
-#define MPCD_PASS_THREADS 256
+#define MPCD_PASS_THREADS 128
 #endif
 constexpr int kPassThreads = MPCD_PASS_THREADS;
 
@@ -77,7 +77,7 @@ __device__ __forceinline__ int w_to_cell(float w) { return __float_as_int(w); }
 __device__ __forceinline__ int w_to_cell(double w) { return (int)__double_as_longlong(w); }
 
 #ifndef MPCD_MINBLOCKS
-#define MPCD_MINBLOCKS 5
+#define MPCD_MINBLOCKS 10     // x 128 threads = 40 warps per SM at <= 51 registers (measured best: DESIGN.md 5.1)
 #endif
 template <typename T, unsigned F>
 __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(const PassArgs<T> a)
