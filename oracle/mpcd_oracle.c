@@ -64,7 +64,7 @@ void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
 }
 
 /* Domain tags (4th counter word), reading A24. */
-enum { DOM_SHIFT = 1, DOM_AXIS = 2, DOM_AT = 3, DOM_INITPOS = 4, DOM_INITVEL = 5 };
+enum { DOM_SHIFT = 1, DOM_AXIS = 2, DOM_AT = 3, DOM_INITPOS = 4, DOM_INITVEL = 5, DOM_THERMO = 6 };
 
 /* Philox(key = seed, ctr = (index, step_lo, step_hi, domain)), reading A24. */
 static void draw_block(uint64_t seed, uint64_t step, uint32_t index, uint32_t domain, uint32_t out[4])
@@ -157,6 +157,52 @@ void oracle_sort_perm(int64_t N, const int32_t *cell, int64_t Nc, int64_t *perm)
     for (int64_t c = 0; c < Nc; ++c) start[c + 1] += start[c];
     for (int64_t i = 0; i < N; ++i) { perm[start[cell[i]]] = i; start[cell[i]] += 1; }
     free(start);
+}
+
+/* ------------------------------------------------------------------------- *
+ * NEXT-2. Maxwell-Boltzmann cell thermostat for SRD (eq. 3,
+ * :157).  Per cell with N_c >= 2: a random kinetic energy E^ is drawn from the
+ * Maxwell-Boltzmann (canonical) distribution of the relative kinetic energy of
+ * N_c particles at kT, i.e. Gamma(shape k = 3 (N_c - 1) / 2, scale kT) (the
+ * N_c - 1 relative velocities have 3 (N_c - 1) quadratic degrees of freedom),
+ * by Marsaglia & Tsang's rejection method (ref. [75]):
+ *     d = k - 1/3, c = 1 / sqrt(9 d);
+ *     repeat: x ~ N(0,1), v = (1 + c x)^3, U ~ U(0,1);
+ *             accept if v > 0 and ln U < x^2/2 + d - d v + d ln v;
+ *     E^ = kT d v.
+ * The Gaussian comes from the Box-Muller transformation of two uniforms
+ * (PAPER.md:157).  xi = sqrt(E^ / E_k); xi = 1 for N_c < 2 (PAPER.md:157:
+ * temperature undefined) and, reading A26, also when E_k = 0.
+ * Reading A26 (paper silent): RNG keyed like the axis, Philox(seed, (cell,
+ * t_lo, t_hi, DOM_THERMO + 256 * iteration)); words 0,1 -> the Gaussian
+ * x = sqrt(-2 ln U0) cos(2 pi U1), word 2 -> U, all by (b + 1/2) 2^-32.
+ * k >= 3/2 always, so the shape < 1 boost of the method is never needed.
+ * ------------------------------------------------------------------------- */
+void oracle_thermostat_xi(uint64_t seed, uint64_t step, int64_t Nc, double kT, const int32_t *count,
+                          const double *erel, double *ehat, double *xi)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int64_t c = 0; c < Nc; ++c) {
+        ehat[c] = 0.0;
+        xi[c] = 1.0;
+        if (count[c] < 2) continue;
+        const double k = 1.5 * (double)(count[c] - 1);
+        const double d = k - 1.0 / 3.0;
+        const double cc = 1.0 / sqrt(9.0 * d);
+        for (uint32_t it = 0;; ++it) {
+            uint32_t b[4];
+            draw_block(seed, step, (uint32_t)c, (uint32_t)DOM_THERMO + 256u * it, b);
+            const double U0 = oracle_u01_32(b[0]), U1 = oracle_u01_32(b[1]), U = oracle_u01_32(b[2]);
+            const double x = sqrt(-2.0 * log(U0)) * cos(two_pi * U1);
+            const double t = 1.0 + cc * x;
+            const double v = t * t * t;
+            if (v > 0.0 && log(U) < 0.5 * x * x + d - d * v + d * log(v)) {
+                ehat[c] = kT * d * v;
+                break;
+            }
+        }
+        if (erel[c] > 0.0) xi[c] = sqrt(ehat[c] / erel[c]);
+    }
 }
 
 /* a4 (count part) + a9 helpers that do not depend on the storage precision. */

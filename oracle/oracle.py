@@ -129,6 +129,23 @@ def collide_srd(vel4, cell, u, axis, alpha):
     getattr(lib(), "oracle_collide_srd" + _suf(vel4.dtype))(C.c_int64(vel4.shape[0]), _p(vel4), _p(cell), _p(u), _p(axis), C.c_double(math.cos(alpha)), C.c_double(math.sin(alpha)))
 
 
+def thermostat_xi(seed, step, kT, count, erel):
+    """NEXT-2: Maxwell-Boltzmann cell thermostat: (E^ per cell, xi per cell)."""
+    Nc = count.shape[0]
+    ehat, xi = np.empty(Nc), np.empty(Nc)
+    lib().oracle_thermostat_xi(C.c_uint64(seed), C.c_uint64(step), C.c_int64(Nc), C.c_double(kT),
+                               _p(np.ascontiguousarray(count, dtype=np.int32)), _p(np.ascontiguousarray(erel, dtype=np.float64)),
+                               _p(ehat), _p(xi))
+    return ehat, xi
+
+
+def collide_srd_xi(vel4, cell, u, axis, xi, alpha):
+    """a6 + Alg. 1 lines 8-10: SRD rotation with the relative velocities scaled by the cell's xi."""
+    getattr(lib(), "oracle_collide_srd_xi" + _suf(vel4.dtype))(
+        C.c_int64(vel4.shape[0]), _p(vel4), _p(cell), _p(u), _p(axis), _p(np.ascontiguousarray(xi, dtype=np.float64)),
+        C.c_double(math.cos(alpha)), C.c_double(math.sin(alpha)))
+
+
 def collide_at(vel4, cell, Nc, count, u, dv):
     """a7: eq. (4), in place on vel4."""
     getattr(lib(), "oracle_collide_at" + _suf(vel4.dtype))(C.c_int64(vel4.shape[0]), _p(vel4), _p(cell), C.c_int64(Nc), _p(count), _p(u), _p(dv))
@@ -170,7 +187,7 @@ class OracleMPCD:
     SRD, AT = 0, 1
 
     def __init__(self, box, N, a=1.0, m=1.0, kT=1.0, seed=0, *, dtype=np.float32, dt=0.1,
-                 alpha=math.radians(130.0), rule=0, sort_period=25, init=True):
+                 alpha=math.radians(130.0), rule=0, sort_period=25, init=True, thermostat=False):
         self.a, self.m, self.kT, self.seed = float(a), float(m), float(kT), int(seed)
         self.n = [int(round(b / a)) for b in box]
         for b, n in zip(box, self.n):
@@ -180,6 +197,8 @@ class OracleMPCD:
         self.N = int(N)
         self.dtype = np.dtype(dtype)
         self.dt, self.alpha, self.rule, self.sort_period = float(dt), float(alpha), int(rule), int(sort_period)
+        self.thermostat = bool(thermostat)
+        self.ehat = self.xi = None
         self.sigma = math.sqrt(self.kT / self.m)
         self.step_count = 0
         if init:
@@ -213,6 +232,8 @@ class OracleMPCD:
         self.count, self.sumv, self.ke = reduce_cells(self.vel, self.cell, self.Nc, self.m)
         self.u, self.erel, self.kTc = finalize_cells(self.vel, self.cell, self.Nc, self.m, self.count, self.sumv)
         self.axis = draw_axis(self.seed, self.step_count, self.Nc)
+        if self.thermostat:      # "we compute xi for each cell at the same time that we draw the rotation vectors"
+            self.ehat, self.xi = thermostat_xi(self.seed, self.step_count, self.kT, self.count, self.erel)
 
     def sort(self):
         perm = sort_perm(self.cell, self.Nc)
@@ -220,7 +241,11 @@ class OracleMPCD:
         return perm
 
     def collide_srd(self, alpha=None):
-        collide_srd(self.vel, self.cell, self.u, self.axis, self.alpha if alpha is None else alpha)
+        alpha = self.alpha if alpha is None else alpha
+        if self.thermostat:
+            collide_srd_xi(self.vel, self.cell, self.u, self.axis, self.xi, alpha)
+        else:
+            collide_srd(self.vel, self.cell, self.u, self.axis, alpha)
 
     def collide_at(self):
         dv = at_draw(self.seed, self.step_count, self.tag, self.sigma)
