@@ -76,7 +76,9 @@ typedef struct mpcd_options {
                               0: momentum and count only (KE is then computed on demand by mpcd_get_cells / thermo) */
     int32_t init_state;    /* 1 (default): draw the initial condition on the device (A23); 0: leave the particle
                               arrays uninitialised, the caller must mpcd_set_state before stepping */
-    int32_t reserved0;
+    int32_t thermostat;    /* 1: Maxwell-Boltzmann cell thermostat for the SRD rule (PAPER.md:45-50 eq. 3, :157): the relative
+                              velocities of every cell with N_c >= 2 are scaled by xi = sqrt(E^/E_k), E^ ~ Gamma(3 (N_c - 1) / 2, kT);
+                              default 0.  Ignored by the AT rule, which is isothermal by construction */
     void *stream;          /* cudaStream_t the library enqueues on; NULL = the legacy default stream */
     mpcd_alloc_fn alloc_fn;
     mpcd_free_fn free_fn;
@@ -159,6 +161,10 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
 
 /* The shift used by the last bin, as applied (mixed mode: the fp32 value, A5).  s: host. */
 int mpcd_get_shift(mpcd_t *h, double s[3]);
+
+/* The thermostat's scale factor xi per cell for the current bin (opt.thermostat = 1; MPCD_ESTATE otherwise or when the
+ * cell sums are not valid).  xi: host, Nc doubles.  Test accessor for the parity of PAPER.md:157. */
+int mpcd_get_xi(mpcd_t *h, double *xi);
 
 /* a9. Net momentum P (3), kinetic energy and pooled temperature (A11) of the
  * CURRENT velocities by device-wide reduction.  If no bin is valid

@@ -27,7 +27,7 @@ FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
 class Options(C.Structure):
     _fields_ = [
         ("precision", C.c_int32), ("rule", C.c_int32), ("dt", C.c_double), ("alpha", C.c_double),
-        ("sort_period", C.c_int32), ("cell_energy", C.c_int32), ("init_state", C.c_int32), ("reserved0", C.c_int32),
+        ("sort_period", C.c_int32), ("cell_energy", C.c_int32), ("init_state", C.c_int32), ("thermostat", C.c_int32),
         ("stream", C.c_void_p), ("alloc_fn", ALLOC_FN), ("free_fn", FREE_FN), ("alloc_user", C.c_void_p),
     ]
 
@@ -50,7 +50,7 @@ EXPORTS = [
     "mpcd_default_options", "mpcd_create", "mpcd_create_ex", "mpcd_destroy", "mpcd_stream", "mpcd_shift_and_bin",
     "mpcd_collide_srd", "mpcd_collide_at", "mpcd_sort", "mpcd_step", "mpcd_get_state", "mpcd_set_state",
     "mpcd_get_cells", "mpcd_get_shift", "mpcd_get_thermo", "mpcd_get_stats", "mpcd_device_ptrs", "mpcd_last_error",
-    "mpcd_abi_version", "mpcd_build_info", "mpcd_test_philox", "mpcd_set_profiling", "mpcd_get_profile",
+    "mpcd_abi_version", "mpcd_build_info", "mpcd_test_philox", "mpcd_set_profiling", "mpcd_get_profile", "mpcd_get_xi",
 ]
 PROF_KINDS = ("fused", "bin", "collide", "cells", "sort", "other", "fused_sort")
 
@@ -79,6 +79,7 @@ def load_library():
     lib.mpcd_set_state.argtypes = [vp, vp, vp, vp, u64]
     lib.mpcd_get_cells.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.mpcd_get_shift.argtypes = [vp, P(dbl)]
+    lib.mpcd_get_xi.argtypes = [vp, vp]
     lib.mpcd_get_thermo.argtypes = [vp, P(dbl), P(dbl), P(dbl)]
     lib.mpcd_get_stats.argtypes = [vp, P(Stats)]
     lib.mpcd_device_ptrs.argtypes = [vp, P(vp), P(vp), P(vp), P(vp)]
@@ -135,7 +136,7 @@ class MPCD:
     """One MPCD solvent on one GPU.  Method names are the C ABI's without the prefix."""
 
     def __init__(self, box, N, a=1.0, m=1.0, kT=1.0, seed=0, *, precision="mixed", rule="srd", dt=0.1,
-                 alpha=math.radians(130.0), sort_period=25, cell_energy=True, init_state=True,
+                 alpha=math.radians(130.0), sort_period=25, cell_energy=True, init_state=True, thermostat=False,
                  device="cuda:0", use_torch_allocator=True, stream=None):
         import torch
         if not torch.cuda.is_available():
@@ -152,6 +153,7 @@ class MPCD:
         opt.rule = MPCD_AT if rule in ("at", MPCD_AT) else MPCD_SRD
         opt.dt, opt.alpha = float(dt), float(alpha)
         opt.sort_period, opt.cell_energy, opt.init_state = int(sort_period), int(bool(cell_energy)), int(bool(init_state))
+        opt.thermostat = int(bool(thermostat))
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         opt.stream = C.c_void_p(self._stream.cuda_stream)
         self._alloc = TorchAllocator(device) if use_torch_allocator else None
@@ -231,6 +233,11 @@ class MPCD:
             o["axis"] = np.empty((Nc, 3))
         self._check(self.lib.mpcd_get_cells(self.h, _ptr(o["count"]), _ptr(o["sumv"]), _ptr(o["ke"]), _ptr(o["u"]), _ptr(o.get("axis")), _ptr(o["kTc"])))
         return o
+
+    def get_xi(self):
+        xi = np.empty(self.Nc)
+        self._check(self.lib.mpcd_get_xi(self.h, _ptr(xi)))
+        return xi
 
     def get_shift(self):
         s = (C.c_double * 3)()

@@ -50,7 +50,7 @@ struct mpcd {
     int num_sms = 148;
     bool debug_sync = false;       // MPCD_DEBUG_SYNC=1: synchronise after every launch (see LAUNCH_CHECK)
     bool zeroed[2] = {false, false}, at_zeroed[2] = {false, false};
-    bool axis_valid[2] = {false, false};
+    bool axis_valid[2] = {false, false}, xi_valid[2] = {false, false};   // xi: the thermostat factor in the axis sector's 4th word
     uint64_t axis_step[2] = {0, 0};
     int max_occ = 0;               // of the last bin whose counts were inspected
     // state machine
@@ -229,6 +229,9 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
         CASE(kSRD | kStream | kBin | kEnergy | kSortOut)
         CASE(kATApply | kStream | kBin | kATDraw | kSortOut)
         CASE(kATApply | kStream | kBin | kATDraw | kEnergy | kSortOut)
+        CASE(kSRD | kThermo)
+        CASE(kSRD | kThermo | kStream | kBin | kEnergy)
+        CASE(kSRD | kThermo | kStream | kBin | kEnergy | kSortOut)
         CASE(kATDraw)
         CASE(kATApply)
 #undef CASE
@@ -272,11 +275,28 @@ int prepare(mpcd_t *h, int zset, bool sums, bool at, bool want_axes, uint64_t ax
     LAUNCH_CHECK(h);
     if (zs) h->zeroed[zset] = true;
     if (za) h->at_zeroed[zset] = true;
-    if (ax) { h->axis_valid[b] = true; h->axis_step[b] = axis_step; }
+    if (ax) { h->axis_valid[b] = true; h->axis_step[b] = axis_step; h->xi_valid[b] = false; }
     return MPCD_OK;
 }
 inline int zero_set(mpcd_t *h, int s, bool sums, bool at) { return prepare(h, s, sums, at, false, 0); }
 inline int ensure_axes(mpcd_t *h, uint64_t t) { return prepare(h, -1, false, false, true, t); }
+
+inline bool thermostatted(const mpcd_t *h) { return h->opt.thermostat != 0; }
+
+// Maxwell-Boltzmann cell thermostat: xi of every cell from the complete sums (incl. energy) of step t in
+// set t & 1, into the 4th word of that step's axis sectors.
+int thermostat(mpcd_t *h, uint64_t t)
+{
+    const int b = (int)(t & 1);
+    if (h->xi_valid[b] && h->axis_valid[b] && h->axis_step[b] == t) return MPCD_OK;
+    int rc = ensure_axes(h, t);
+    if (rc) return rc;
+    ProfScope prof(h, MPCD_PROF_CELLS);
+    cell_thermostat<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[b], h->qacc[b], h->axis[b], h->Nc, h->m, h->kT, h->seed, t);
+    LAUNCH_CHECK(h);
+    h->xi_valid[b] = true;
+    return MPCD_OK;
+}
 
 // a8, first half: exclusive scan of the per-cell counts of accumulator set `s` -> cell_start (the write cursors)
 int scan_counts(mpcd_t *h, int s)
@@ -338,6 +358,7 @@ int bin_accumulate(mpcd_t *h, uint64_t t)
     h->ccur = set;
     h->bin_valid = true; h->bin_step = t;
     rc = ensure_axes(h, t);
+    if (!rc && thermostatted(h)) rc = thermostat(h, t);
     if (rc) return rc;
     h->sums_valid = true; h->energy_valid = true; h->counts_valid = true;
     return MPCD_OK;
@@ -432,6 +453,7 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
     if (opt) o = *opt;
     if (o.precision != MPCD_MIXED && o.precision != MPCD_FP64) return fail(nullptr, MPCD_EINVAL, "bad precision%s");
     if (o.rule != MPCD_SRD && o.rule != MPCD_AT) return fail(nullptr, MPCD_EINVAL, "bad rule%s");
+    if (o.thermostat != 0 && o.thermostat != 1) return fail(nullptr, MPCD_EINVAL, "thermostat must be 0 or 1%s");
     if (!(o.dt > 0) || o.sort_period < 0) return fail(nullptr, MPCD_EINVAL, "dt must be > 0 and sort_period >= 0%s");
     if ((o.alloc_fn == nullptr) != (o.free_fn == nullptr)) return fail(nullptr, MPCD_EINVAL, "alloc_fn and free_fn must be given together%s");
     int32_t n[3];
@@ -523,12 +545,13 @@ int mpcd_collide_srd(mpcd_t *h, double alpha)
     if (!(h->bin_valid && h->bin_step == h->step && h->sums_valid))
         return fail(h, MPCD_ESTATE, "collide_srd needs mpcd_shift_and_bin for the current step first%s");
     int rc = ensure_axes(h, h->step);
+    if (!rc && thermostatted(h)) rc = h->energy_valid ? thermostat(h, h->step) : fail(h, MPCD_ESTATE, "thermostat needs the cell energies%s");
     if (rc) return rc;
     PassPlan pl;
     pl.cset = pl.bset = h->ccur;
     pl.step_collide = pl.step_bin = h->step;
     pl.alpha = alpha;
-    rc = pass(h, kSRD, pl);
+    rc = pass(h, kSRD | (thermostatted(h) ? kThermo : 0u), pl);
     if (rc) return rc;
     h->sums_valid = false; h->energy_valid = false;
     return MPCD_OK;
@@ -569,7 +592,8 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     if (nsteps < 0) return fail(h, MPCD_EINVAL, "nsteps must be >= 0%s");
     if (nsteps == 0) return MPCD_OK;
     const bool at = h->opt.rule == MPCD_AT;
-    const unsigned fe = h->opt.cell_energy != 0 ? kEnergy : 0u;
+    const unsigned ft = (!at && thermostatted(h)) ? kThermo : 0u;
+    const unsigned fe = (h->opt.cell_energy != 0 || ft) ? kEnergy : 0u;      // the thermostat needs the cell energies
     int rc = at ? ensure_at_buffers(h) : MPCD_OK;
     if (rc) return rc;
     uint64_t t = h->step;
@@ -585,6 +609,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
     rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), pl);
     if (rc) return rc;
+    if (ft) { rc = thermostat(h, t); if (rc) return rc; }
     bool sort_pending = sort_due(h, t);            // sort by the cells of step t: done by the next fused kernel on its way out
     // steady state, two launches per step: cell_prepare (zeroed set and axes of step t + 1), then collide(t) fused with
     // stream + bin + accumulate (t + 1)
@@ -597,17 +622,18 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
         pl.cset = set; pl.bset = nxt;
         pl.step_collide = t; pl.step_bin = t + 1;
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
-        rc = pass(h, (at ? (kATApply | kATDraw) : kSRD) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
+        rc = pass(h, (at ? (kATApply | kATDraw) : (kSRD | ft)) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
         if (rc) return rc;
         if (sort_pending) { h->pcur ^= 1; h->sorts += 1; }
         set = nxt; t += 1;
+        if (ft) { rc = thermostat(h, t); if (rc) return rc; }
         sort_pending = sort_due(h, t);
     }
     if (sort_pending) { rc = do_sort(h, set); if (rc) return rc; }
     // last collision
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;
-    rc = pass(h, at ? kATApply : kSRD, pl);
+    rc = pass(h, at ? kATApply : (kSRD | ft), pl);
     if (rc) return rc;
     h->ccur = set;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = pl.shift[d];
@@ -682,6 +708,19 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
     if (cudaStreamSynchronize(h->stream) != cudaSuccess && rc == MPCD_OK) rc = fail(h, MPCD_ECUDA, "get_cells sync failed%s");
     cudaFree(tmp);
     return rc;
+}
+
+int mpcd_get_xi(mpcd_t *h, double *xi)
+{
+    if (!h || !xi) return MPCD_EINVAL;
+    if (!thermostatted(h)) return fail(h, MPCD_ESTATE, "the thermostat is off (opt.thermostat)%s");
+    if (!(h->bin_valid && h->sums_valid && h->energy_valid)) return fail(h, MPCD_ESTATE, "cell sums are not valid: call mpcd_shift_and_bin first%s");
+    int rc = thermostat(h, h->bin_step);
+    if (rc) return rc;
+    CUDA_TRY(h, cudaMemcpy2DAsync(xi, sizeof(double), h->axis[h->bin_step & 1] + 3, 4 * sizeof(double), sizeof(double), (size_t)h->Nc,
+                                  cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return MPCD_OK;
 }
 
 int mpcd_get_shift(mpcd_t *h, double s[3])

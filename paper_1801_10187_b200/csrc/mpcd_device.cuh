@@ -13,7 +13,7 @@ namespace mpcdk {
 // Counter-based RNG: Philox4x32-10 keyed like the paper keys Saru, (cell index | tag,
 // timestep, seed) (A24): key = seed, ctr = (index, t_lo, t_hi, domain).
 // ---------------------------------------------------------------------------------------
-enum : uint32_t { kDomShift = 1u, kDomAxis = 2u, kDomAT = 3u, kDomInitPos = 4u, kDomInitVel = 5u };
+enum : uint32_t { kDomShift = 1u, kDomAxis = 2u, kDomAT = 3u, kDomInitPos = 4u, kDomInitVel = 5u, kDomThermo = 6u };
 
 struct u32x4 { uint32_t x, y, z, w; };
 
@@ -70,6 +70,23 @@ __device__ __forceinline__ void gauss3_from_block(const u32x4 b, double &g0, dou
 __device__ __forceinline__ void draw_gauss3(uint64_t seed, uint64_t step, uint32_t tag, double &g0, double &g1, double &g2)
 {
     gauss3_from_block(draw(seed, step, tag, kDomAT), g0, g1, g2);
+}
+
+// Maxwell-Boltzmann cell thermostat (A26): the relative kinetic energy of a cell of n >= 2
+// particles at kT, drawn from Gamma(shape 3 (n - 1) / 2, scale kT) by Marsaglia & Tsang's rejection method with a
+// Box-Muller Gaussian; one Philox block per attempt, keyed (seed, step, cell, kDomThermo + 256 * attempt).
+__device__ __forceinline__ double draw_cell_energy(uint64_t seed, uint64_t step, uint32_t cell, int n, double kT)
+{
+    const double k = 1.5 * (double)(n - 1);
+    const double d = k - 1.0 / 3.0;
+    const double c = 1.0 / sqrt(9.0 * d);
+    for (uint32_t attempt = 0;; ++attempt) {
+        const u32x4 b = draw(seed, step, cell, kDomThermo + 256u * attempt);
+        const double x = sqrt(-2.0 * log(u01_32(b.x))) * cospi(2.0 * u01_32(b.y));
+        const double t = 1.0 + c * x;
+        const double v = t * t * t;
+        if (v > 0.0 && log(u01_32(b.z)) < 0.5 * x * x + d - d * v + d * log(v)) return kT * d * v;
+    }
 }
 
 // ---------------------------------------------------------------------------------------

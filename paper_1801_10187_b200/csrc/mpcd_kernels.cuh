@@ -10,6 +10,8 @@
 //   kBin      a3+a4  shifted binning + fp64 cell accumulation
 //   kEnergy   a4     also accumulate sum |v|^2 (kinetic energy, eq. 3)
 //   kATDraw   a7     draw dv for the (new) step and accumulate its per-cell sum
+//   kThermo   a6     with kSRD: scale the rotated relative velocity by the cell's xi (Maxwell-Boltzmann cell thermostat,
+//                    Alg. 1 lines 8-10 PAPER.md:150-152); xi rides in the 4th word of the cell's axis sector
 //   kSortOut  a8     sort by cell on the way out: instead of in place, the particle is written
 //                    to slot cell_start[c] + (atomic cursor) of the duplicate arrays, c = its cell in the step
 //                    being collided; the separate read-and-scatter pass of the sort disappears
@@ -24,7 +26,7 @@
 
 namespace mpcdk {
 
-enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u };
+enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u };
 
 template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
@@ -119,7 +121,8 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
             const double rx = wx * a.cos_a + (n.y * wz - n.z * wy) * a.sin_a + n.x * ndw * omc;
             const double ry = wy * a.cos_a + (n.z * wx - n.x * wz) * a.sin_a + n.y * ndw * omc;
             const double rz = wz * a.cos_a + (n.x * wy - n.y * wx) * a.sin_a + n.z * ndw * omc;
-            v.x = (T)(ux + rx); v.y = (T)(uy + ry); v.z = (T)(uz + rz);                          // lines 11-12
+            const double xi = (F & kThermo) ? n.w : 1.0;                                        // lines 8-10
+            v.x = (T)(ux + rx * xi); v.y = (T)(uy + ry * xi); v.z = (T)(uz + rz * xi);           // lines 11-12
         }
     }
     if (F & kATApply) {
@@ -183,6 +186,26 @@ __global__ void __launch_bounds__(256) cell_prepare(double *axis, uint64_t seed,
         draw_axis(seed, step, (uint32_t)c, nx, ny, nz);
         st256(axis + 4 * c, nx, ny, nz, 0.0);
     }
+}
+
+// Maxwell-Boltzmann cell thermostat: once the sums of a step are complete, the scale factor
+// xi = sqrt(E^ / E_k) of every cell, E_k = m (sum |v|^2 - |S|^2 / N_c) / 2 (eq. 3; A12), E^ drawn
+// from the canonical distribution; xi = 1 for N_c < 2 and for E_k = 0.  Written into the 4th word of the cell's
+// axis sector, which the collision gathers anyway.
+__global__ void __launch_bounds__(256) cell_thermostat(const double *acc, const double *qacc, double *axis, int64_t Nc, double m, double kT,
+                                                       uint64_t seed, uint64_t step)
+{
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= Nc) return;
+    const f64x4 s = ld256(acc + 4 * c);
+    const int n = (int)s.w;
+    double xi = 1.0;
+    if (n >= 2) {
+        const double erel = 0.5 * m * (qacc[c] - (s.x * s.x + s.y * s.y + s.z * s.z) / s.w);
+        const double ehat = draw_cell_energy(seed, step, (uint32_t)c, n, kT);
+        if (erel > 0.0) xi = sqrt(ehat / erel);
+    }
+    axis[4 * c + 3] = xi;
 }
 
 // Largest cell occupancy of a bin (mpcd_get_stats), from the counts in the accumulator set.

@@ -1,0 +1,81 @@
+"""GPU parity for the Maxwell-Boltzmann cell thermostat through
+the C ABI: the scale factors xi against the oracle's, velocities after thermostatted steps within the
+north_star tolerance, and the invariants (temperature reaches kT within statistical error, momentum kept)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1801_10187_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def _pair(oracle, n, M, seed, dtype, kT=1.0, kT_init=None, **kw):
+    from paper_1801_10187_b200 import MPCD
+    pos, vel, tag = synth.solvent(n, M, seed=seed, kT=kT if kT_init is None else kT_init, dtype=dtype)
+    box = [float(x) for x in n]
+    g = MPCD(box, pos.shape[0], kT=kT, seed=seed, precision="fp64" if dtype == np.float64 else "mixed", init_state=False,
+             thermostat=True, **kw)
+    g.set_state(pos, vel, tag)
+    o = oracle.OracleMPCD(box, pos.shape[0], kT=kT, seed=seed, dtype=dtype, init=False, thermostat=True, **kw)
+    o.set_state(pos, vel, tag)
+    return g, o
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_scale_factors_and_one_collision_match_the_oracle(oracle, dtype):
+    g, o = _pair(oracle, (12, 9, 7), 6, 21, dtype, kT=0.8)
+    g.stream(); o.stream()
+    g.shift_and_bin(); o.shift_and_bin()
+    xi = g.get_xi()
+    small = o.count < 2
+    assert np.all(xi[small] == 1.0)
+    np.testing.assert_allclose(xi, o.xi, rtol=1e-9)                         # E_k by one pass (A12) vs the oracle's two passes
+    g.collide_srd(math.radians(130.0)); o.collide_srd(math.radians(130.0))
+    gv = g.get_state()["vel"][:, :3].astype(np.float64)
+    tol = 1e-12 if dtype == np.float64 else 1e-5
+    assert np.max(np.abs(gv - o.vel[:, :3].astype(np.float64))) <= tol * max(1.0, float(np.max(xi)))
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_fused_thermostatted_steps_match_the_oracle(oracle, dtype):
+    g, o = _pair(oracle, (10, 10, 8), 10, 8, dtype, sort_period=2)
+    g.step(3); o.step(3)
+    s = g.get_state()
+    a, b = np.argsort(s["tag"]), np.argsort(o.tag)
+    ptol = 1e-6 if dtype == np.float32 else 1e-12
+    assert np.max(np.abs(s["pos"][a][:, :3].astype(np.float64) - o.pos[b][:, :3])) <= ptol
+    assert np.array_equal(s["cell"][a], o.cell[b])
+    err = np.max(np.abs(s["vel"][a][:, :3].astype(np.float64) - o.vel[b][:, :3].astype(np.float64)))
+    assert err <= 3 * (1e-12 if dtype == np.float64 else 1e-5), err
+
+
+def test_thermostat_brings_a_hot_fluid_to_kT_and_keeps_momentum():
+    from paper_1801_10187_b200 import MPCD
+    n, M, kT = (48, 48, 48), 10, 1.0
+    pos, vel, tag = synth.solvent(n, M, seed=3, kT=2.5, dtype=np.float32)
+    N = pos.shape[0]
+    g = MPCD([float(x) for x in n], N, kT=kT, seed=3, init_state=False, thermostat=True)
+    g.set_state(pos, vel, tag)
+    P0, _, kT0 = g.get_thermo()
+    assert abs(kT0 - 2.5) < 0.02
+    dof = 1.5 * (N - n[0] * n[1] * n[2])                # ~ sum over cells of 1.5 (N_c - 1)
+    kTs = []
+    for _ in range(6):
+        g.step(5)
+        P, _, k = g.get_thermo()
+        kTs.append(k)
+        assert np.max(np.abs(P - P0)) / N <= 1e-6
+    assert all(abs(k - kT) <= 6 * kT / math.sqrt(dof) + 2e-4 for k in kTs), kTs     # re-binning adds ~2e-4 (see test_gpu_fullsize)
+    g.close()
+
+
+def test_thermostat_off_has_no_xi():
+    from paper_1801_10187_b200 import MPCD, MPCDError
+    g = MPCD([4.0, 4.0, 4.0], 640, seed=1)
+    g.shift_and_bin()
+    with pytest.raises(MPCDError) as e:
+        g.get_xi()
+    assert e.value.code == -4
+    g.close()
