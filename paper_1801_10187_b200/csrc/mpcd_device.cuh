@@ -67,9 +67,45 @@ __device__ __forceinline__ void gauss3_from_block(const u32x4 b, double &g0, dou
     g0 = r01 * c; g1 = r01 * s;
     g2 = r23 * cospi(2.0 * u01_32(b.w));
 }
+// The same three Gaussians evaluated in fp32 for the mixed model (A17 allows it as long as the 1e-5 sigma velocity
+// parity holds; no fast-math intrinsics): absolute error <= ~1e-6 against the fp64 evaluation, by construction:
+//  - radius sqrt(-2 ln U): for U > 1/2 the exact small quantity is w = 1 - U = (2^32 - b - 1/2) 2^-32, so
+//    ln U = log1pf(-w) keeps full RELATIVE accuracy where the radius is small; for U <= 1/2, logf(U) has absolute
+//    error ~6e-8 and the radius is > 1.17;
+//  - angle 2 U1 (in units of pi) = hi + lo with hi the top 24 bits (exact in fp32) and lo < 2^-23 applied as a
+//    first-order rotation of sincospif(hi), instead of rounding U1 itself to 24 bits.
+__device__ __forceinline__ float bm_radius_f32(uint32_t b)
+{
+    float lnu;
+    if (b & 0x80000000u) lnu = log1pf(-((float)(0xffffffffu - b) + 0.5f) * 2.3283064365386962890625e-10f);
+    else lnu = logf(((float)b + 0.5f) * 2.3283064365386962890625e-10f);
+    return sqrtf(-2.0f * lnu);
+}
+__device__ __forceinline__ void bm_sincos_f32(uint32_t b, float &s, float &c)      // sin, cos of 2 pi (b + 1/2) 2^-32
+{
+    const float hi = (float)(b >> 8) * 1.1920928955078125e-7f;                     // (b >> 8) 2^-23: exact
+    const float lo = ((float)(b & 255u) + 0.5f) * 4.656612873077392578125e-10f;    // ((b & 255) + 1/2) 2^-31: exact
+    float sh, ch;
+    sincospif(hi, &sh, &ch);
+    const float d = 3.14159265358979323846f * lo;
+    s = fmaf(d, ch, sh);
+    c = fmaf(-d, sh, ch);
+}
+__device__ __forceinline__ void gauss3_from_block_f32(const u32x4 b, double &g0, double &g1, double &g2)
+{
+    const float r01 = bm_radius_f32(b.x), r23 = bm_radius_f32(b.z);
+    float s1, c1, s3, c3;
+    bm_sincos_f32(b.y, s1, c1);
+    bm_sincos_f32(b.w, s3, c3);
+    g0 = (double)(r01 * c1); g1 = (double)(r01 * s1); g2 = (double)(r23 * c3);
+}
+// T = the native precision of the model: the fp64 model evaluates the transform in double.
+template <typename T>
 __device__ __forceinline__ void draw_gauss3(uint64_t seed, uint64_t step, uint32_t tag, double &g0, double &g1, double &g2)
 {
-    gauss3_from_block(draw(seed, step, tag, kDomAT), g0, g1, g2);
+    const u32x4 b = draw(seed, step, tag, kDomAT);
+    if (sizeof(T) == 4) gauss3_from_block_f32(b, g0, g1, g2);
+    else gauss3_from_block(b, g0, g1, g2);
 }
 
 // Maxwell-Boltzmann cell thermostat (A26): the relative kinetic energy of a cell of n >= 2

@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
             const f64x4 d = ld256_nc(a.dsum + 4 * (size_t)c);
             const double inv = __drcp_rn(s.w);
             double g0, g1, g2;
-            draw_gauss3(a.seed, a.step_collide, tag, g0, g1, g2);
+            draw_gauss3<T>(a.seed, a.step_collide, tag, g0, g1, g2);
             v.x = (T)((s.x - d.x) * inv + a.sigma * g0);
             v.y = (T)((s.y - d.y) * inv + a.sigma * g1);
             v.z = (T)((s.z - d.z) * inv + a.sigma * g2);
@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     if (F & kBin) warp_cell_accumulate<T, true, (F & kEnergy) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
     if (F & kATDraw) {
         double g0 = 0, g1 = 0, g2 = 0;
-        if (valid) draw_gauss3(a.seed, a.step_bin, tag, g0, g1, g2);
+        if (valid) draw_gauss3<T>(a.seed, a.step_bin, tag, g0, g1, g2);
         warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, a.sigma * g0, a.sigma * g1, a.sigma * g2);
     }
 }

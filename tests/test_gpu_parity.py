@@ -159,9 +159,12 @@ def test_fused_step_equals_oracle_steps(oracle, dtype, rule):
     gs = _by_tag(g.get_state())
     os_ = np.argsort(o.tag)
     assert gs["step"] == 3 and np.array_equal(gs["tag"], o.tag[os_])
-    ptol = 1e-6 if dtype == np.float32 else 1e-12
+    # mixed model: a velocity that differs within the tolerance moves a later position by an fp32 ulp or two
+    # (ulp(16) = 9.5e-7; the AT rule's fp32 Box-Muller transform, reading A17, differs from the oracle's fp64 one by
+    # up to 7e-7), and a position within an ulp of a cell boundary may then bin differently
+    ptol = 4e-6 if dtype == np.float32 else 1e-12
     assert np.max(np.abs(gs["pos"][:, :3].astype(np.float64) - o.pos[os_][:, :3])) <= ptol
-    assert np.array_equal(gs["cell"], o.cell[os_])
+    assert np.count_nonzero(gs["cell"] != o.cell[os_]) <= (2 if dtype == np.float32 else 0)
     err = np.max(np.abs(gs["vel"][:, :3].astype(np.float64) - o.vel[os_][:, :3].astype(np.float64)))
     assert err <= 3 * _tol(dtype), err
 
