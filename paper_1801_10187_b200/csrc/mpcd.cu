@@ -232,6 +232,13 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
         CASE(kSRD | kThermo)
         CASE(kSRD | kThermo | kStream | kBin | kEnergy)
         CASE(kSRD | kThermo | kStream | kBin | kEnergy | kSortOut)
+        CASE(kStream | kBin | kATDraw | kATStored)
+        CASE(kStream | kBin | kATDraw | kEnergy | kATStored)
+        CASE(kATApply | kStream | kBin | kATDraw | kATStored)
+        CASE(kATApply | kStream | kBin | kATDraw | kEnergy | kATStored)
+        CASE(kATApply | kStream | kBin | kATDraw | kATStored | kSortOut)
+        CASE(kATApply | kStream | kBin | kATDraw | kEnergy | kATStored | kSortOut)
+        CASE(kATApply | kATStored)
         CASE(kATDraw)
         CASE(kATApply)
 #undef CASE
@@ -607,7 +614,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
-    rc = pass(h, kStream | kBin | fe | (at ? kATDraw : 0u), pl);
+    rc = pass(h, kStream | kBin | fe | (at ? (kATDraw | kATStored) : 0u), pl);   // AT: vel.xyz carries dv between the launches of this call
     if (rc) return rc;
     if (ft) { rc = thermostat(h, t); if (rc) return rc; }
     bool sort_pending = sort_due(h, t);            // sort by the cells of step t: done by the next fused kernel on its way out
@@ -622,7 +629,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
         pl.cset = set; pl.bset = nxt;
         pl.step_collide = t; pl.step_bin = t + 1;
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
-        rc = pass(h, (at ? (kATApply | kATDraw) : (kSRD | ft)) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
+        rc = pass(h, (at ? (kATApply | kATDraw | kATStored) : (kSRD | ft)) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
         if (rc) return rc;
         if (sort_pending) { h->pcur ^= 1; h->sorts += 1; }
         set = nxt; t += 1;
@@ -633,7 +640,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     // last collision
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;
-    rc = pass(h, at ? kATApply : (kSRD | ft), pl);
+    rc = pass(h, at ? (kATApply | kATStored) : (kSRD | ft), pl);
     if (rc) return rc;
     h->ccur = set;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = pl.shift[d];

@@ -12,6 +12,9 @@
 //   kATDraw   a7     draw dv for the (new) step and accumulate its per-cell sum
 //   kThermo   a6     with kSRD: scale the rotated relative velocity by the cell's xi (Maxwell-Boltzmann cell thermostat,
 //                    Alg. 1 lines 8-10 PAPER.md:150-152); xi rides in the 4th word of the cell's axis sector
+//   kATStored a7     inside mpcd_step: kATDraw leaves the drawn dv in vel.xyz instead of the velocity (the AT update
+//                    v = u + dv - D/N_c does not depend on the old velocity, which has been summed by then), and the
+//                    next kATApply takes it from there instead of regenerating it: one Gaussian draw per particle-step
 //   kSortOut  a8     sort by cell on the way out: instead of in place, the particle is written
 //                    to slot cell_start[c] + (atomic cursor) of the duplicate arrays, c = its cell in the step
 //                    being collided; the separate read-and-scatter pass of the sort disappears
@@ -26,7 +29,7 @@
 
 namespace mpcdk {
 
-enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u };
+enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u };
 
 template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
@@ -104,7 +107,7 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     if (valid) {
         v = load4(a.vel + i);
         if (F & (kStream | kBin)) p = load4(a.pos + i);
-        if (F & (kATApply | kATDraw | kSortOut)) tag = a.tag[i];
+        if ((F & (kATDraw | kSortOut)) || ((F & kATApply) && !(F & kATStored))) tag = a.tag[i];
     }
     int c = valid ? w_to_cell(v.w) : inactive;                   // cell of the last binning (the step being collided)
     int64_t o = i;                                               // where this particle is written
@@ -130,11 +133,17 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
             const f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);
             const f64x4 d = ld256_nc(a.dsum + 4 * (size_t)c);
             const double inv = __drcp_rn(s.w);
-            double g0, g1, g2;
-            draw_gauss3<T>(a.seed, a.step_collide, tag, g0, g1, g2);
-            v.x = (T)((s.x - d.x) * inv + a.sigma * g0);
-            v.y = (T)((s.y - d.y) * inv + a.sigma * g1);
-            v.z = (T)((s.z - d.z) * inv + a.sigma * g2);
+            double dx, dy, dz;                                   // dv_i of the step being collided
+            if (F & kATStored) {
+                dx = (double)v.x; dy = (double)v.y; dz = (double)v.z;
+            } else {
+                double g0, g1, g2;
+                draw_gauss3<T>(a.seed, a.step_collide, tag, g0, g1, g2);
+                dx = a.sigma * g0; dy = a.sigma * g1; dz = a.sigma * g2;
+            }
+            v.x = (T)((s.x - d.x) * inv + dx);
+            v.y = (T)((s.y - d.y) * inv + dy);
+            v.z = (T)((s.z - d.z) * inv + dz);
         }
     }
     if (F & kStream) {
@@ -149,14 +158,23 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
         c = valid ? cell_of<T>(p, a.shift, a.inv_a, a.n) : inactive;
         v.w = cell_to_w(c, T(0));
     }
-    if ((F & (kSRD | kATApply | kBin)) && valid) store4(((F & kSortOut) ? a.vel_out : a.vel) + o, v);
+    V4 vs = v;                                                   // what goes back to the velocity array
+    double ex = 0, ey = 0, ez = 0;                               // dv_i of the step being binned
+    if (F & kATDraw) {
+        if (valid) {
+            double g0, g1, g2;
+            draw_gauss3<T>(a.seed, a.step_bin, tag, g0, g1, g2);
+            ex = a.sigma * g0; ey = a.sigma * g1; ez = a.sigma * g2;
+            if (F & kATStored) {                                 // the sum below must be the sum of what is stored
+                vs.x = (T)ex; vs.y = (T)ey; vs.z = (T)ez;
+                ex = (double)vs.x; ey = (double)vs.y; ez = (double)vs.z;
+            }
+        }
+    }
+    if ((F & (kSRD | kATApply | kBin)) && valid) store4(((F & kSortOut) ? a.vel_out : a.vel) + o, vs);
     if ((F & kSortOut) && valid) a.tag_out[o] = tag;
     if (F & kBin) warp_cell_accumulate<T, true, (F & kEnergy) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
-    if (F & kATDraw) {
-        double g0 = 0, g1 = 0, g2 = 0;
-        if (valid) draw_gauss3<T>(a.seed, a.step_bin, tag, g0, g1, g2);
-        warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, a.sigma * g0, a.sigma * g1, a.sigma * g2);
-    }
+    if (F & kATDraw) warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, ex, ey, ez);
 }
 
 // Cell index of every particle (the cache in vel.w) as an int32 array, on demand (mpcd_get_state, mpcd_device_ptrs).
