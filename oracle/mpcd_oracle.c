@@ -205,6 +205,93 @@ void oracle_thermostat_xi(uint64_t seed, uint64_t step, int64_t Nc, double kT, c
     }
 }
 
+/* ------------------------------------------------------------------------- *
+ * NEXT-1. Embedded solute (BASELINE config 5): MD beads that
+ * take part in the collision.  Beads are kept in double whatever the solvent's
+ * storage precision (reading A27: there are few of them), as nb x 3 arrays.
+ *
+ * Between collisions the beads follow "the standard MD equations of motion ...
+ * using the velocity Verlet algorithm".  The only forces here are
+ * harmonic bonds U = k (r - r0)^2 / 2 between consecutive beads of a linear chain
+ * of chain_len beads (config 5; the paper's own polymer model, ref. [78], is not
+ * specified in PAPER.md), with the minimum-image convention.
+ * ------------------------------------------------------------------------- */
+void oracle_md_forces(int64_t nb, int32_t chain_len, const double *pos3, double k, double r0, const double L[3], double *f3)
+{
+    for (int64_t i = 0; i < 3 * nb; ++i) f3[i] = 0.0;
+    for (int64_t i = 0; i + 1 < nb; ++i) {
+        if ((i + 1) % chain_len == 0) continue;                 /* i is the last bead of its chain */
+        double d[3], r2 = 0.0;
+        for (int a = 0; a < 3; ++a) {
+            d[a] = pos3[3 * (i + 1) + a] - pos3[3 * i + a];
+            d[a] -= L[a] * floor(d[a] / L[a] + 0.5);            /* minimum image */
+            r2 += d[a] * d[a];
+        }
+        const double r = sqrt(r2);
+        const double g = r > 0.0 ? -k * (r - r0) / r : 0.0;     /* force on bead i+1 = g d, on bead i = -g d */
+        for (int a = 0; a < 3; ++a) { f3[3 * (i + 1) + a] += g * d[a]; f3[3 * i + a] -= g * d[a]; }
+    }
+}
+
+/* nsub velocity-Verlet steps of length dt: v += f dt / 2m; x += v dt (wrapped into [0, L)); f = F(x); v += f dt / 2m. */
+void oracle_md_verlet(int64_t nb, int32_t chain_len, double *pos3, double *vel3, const double *mass, double k, double r0,
+                      const double L[3], double dt, int32_t nsub)
+{
+    double *f = (double *)malloc((size_t)nb * 3 * sizeof(double));
+    oracle_md_forces(nb, chain_len, pos3, k, r0, L, f);
+    for (int s = 0; s < nsub; ++s) {
+        for (int64_t i = 0; i < nb; ++i)
+            for (int a = 0; a < 3; ++a) {
+                vel3[3 * i + a] += 0.5 * dt * f[3 * i + a] / mass[i];
+                double x = pos3[3 * i + a] + vel3[3 * i + a] * dt;
+                if (x < 0.0) x += L[a];
+                if (x >= L[a]) x -= L[a];
+                pos3[3 * i + a] = x;
+            }
+        oracle_md_forces(nb, chain_len, pos3, k, r0, L, f);
+        for (int64_t i = 0; i < nb; ++i)
+            for (int a = 0; a < 3; ++a) vel3[3 * i + a] += 0.5 * dt * f[3 * i + a] / mass[i];
+    }
+    free(f);
+}
+
+/* Mass-weighted cell mean with embedded particles ("the MD particles ... included in the collision step",
+ * :159; reading A10): u = (m sum_solvent v + sum_beads m_b v_b) / (m N_solvent + sum_beads m_b). */
+void oracle_embedded_means(int64_t Nc, double m, const int32_t *count, const double *sumv3, int64_t nb, const int32_t *cell_b,
+                           const double *vel3_b, const double *mass_b, double *u3, double *Mc)
+{
+    double *P = (double *)calloc((size_t)Nc * 3, sizeof(double));
+    for (int64_t c = 0; c < Nc; ++c) {
+        Mc[c] = m * (double)count[c];
+        for (int a = 0; a < 3; ++a) P[3 * c + a] = m * sumv3[3 * c + a];
+    }
+    for (int64_t i = 0; i < nb; ++i) {
+        const int64_t c = cell_b[i];
+        Mc[c] += mass_b[i];
+        for (int a = 0; a < 3; ++a) P[3 * c + a] += mass_b[i] * vel3_b[3 * i + a];
+    }
+    for (int64_t c = 0; c < Nc; ++c)
+        for (int a = 0; a < 3; ++a) u3[3 * c + a] = Mc[c] > 0.0 ? P[3 * c + a] / Mc[c] : 0.0;
+    free(P);
+}
+
+/* SRD rotation of the beads about their cell's axis, relative to the (mass-weighted) cell mean: eq. (2), Alg. 1. */
+void oracle_collide_srd_beads(int64_t nb, double *vel3, const int32_t *cell_b, const double *u3, const double *axis3,
+                              double cos_a, double sin_a)
+{
+    for (int64_t i = 0; i < nb; ++i) {
+        const int64_t c = cell_b[i];
+        const double ux = u3[3 * c], uy = u3[3 * c + 1], uz = u3[3 * c + 2];
+        const double nx = axis3[3 * c], ny = axis3[3 * c + 1], nz = axis3[3 * c + 2];
+        const double wx = vel3[3 * i] - ux, wy = vel3[3 * i + 1] - uy, wz = vel3[3 * i + 2] - uz;
+        const double ndw = nx * wx + ny * wy + nz * wz;
+        const double cx = ny * wz - nz * wy, cy = nz * wx - nx * wz, cz = nx * wy - ny * wx;
+        vel3[3 * i + 0] = ux + wx * cos_a + cx * sin_a + nx * ndw * (1.0 - cos_a);
+        vel3[3 * i + 1] = uy + wy * cos_a + cy * sin_a + ny * ndw * (1.0 - cos_a);
+        vel3[3 * i + 2] = uz + wz * cos_a + cz * sin_a + nz * ndw * (1.0 - cos_a);
+    }
+}
+
 /* a4 (count part) + a9 helpers that do not depend on the storage precision. */
 
 /* a9. Net momentum, kinetic energy and pooled temperature from the cell arrays

@@ -146,6 +146,34 @@ def collide_srd_xi(vel4, cell, u, axis, xi, alpha):
         C.c_double(math.cos(alpha)), C.c_double(math.sin(alpha)))
 
 
+def md_forces(pos3, chain_len, k, r0, L):
+    """NEXT-1: harmonic bond forces on the beads of linear chains (minimum image)."""
+    f = np.empty_like(pos3)
+    lib().oracle_md_forces(C.c_int64(pos3.shape[0]), C.c_int32(chain_len), _p(pos3), C.c_double(k), C.c_double(r0), _d3(L), _p(f))
+    return f
+
+
+def md_verlet(pos3, vel3, mass, chain_len, k, r0, L, dt, nsub):
+    """NEXT-1: nsub velocity-Verlet steps of the beads, in place."""
+    assert pos3.dtype == np.float64 and vel3.dtype == np.float64 and mass.dtype == np.float64
+    lib().oracle_md_verlet(C.c_int64(pos3.shape[0]), C.c_int32(chain_len), _p(pos3), _p(vel3), _p(mass), C.c_double(k), C.c_double(r0),
+                           _d3(L), C.c_double(dt), C.c_int32(nsub))
+
+
+def embedded_means(m, count, sumv, cell_b, vel3_b, mass_b):
+    """NEXT-1: mass-weighted cell mean velocity and cell mass with embedded beads."""
+    Nc = count.shape[0]
+    u, Mc = np.empty((Nc, 3)), np.empty(Nc)
+    lib().oracle_embedded_means(C.c_int64(Nc), C.c_double(m), _p(count), _p(sumv), C.c_int64(cell_b.shape[0]), _p(cell_b), _p(vel3_b),
+                                _p(mass_b), _p(u), _p(Mc))
+    return u, Mc
+
+
+def collide_srd_beads(vel3, cell_b, u, axis, alpha):
+    lib().oracle_collide_srd_beads(C.c_int64(vel3.shape[0]), _p(vel3), _p(cell_b), _p(u), _p(axis), C.c_double(math.cos(alpha)),
+                                   C.c_double(math.sin(alpha)))
+
+
 def collide_at(vel4, cell, Nc, count, u, dv):
     """a7: eq. (4), in place on vel4."""
     getattr(lib(), "oracle_collide_at" + _suf(vel4.dtype))(C.c_int64(vel4.shape[0]), _p(vel4), _p(cell), C.c_int64(Nc), _p(count), _p(u), _p(dv))
@@ -199,6 +227,7 @@ class OracleMPCD:
         self.dt, self.alpha, self.rule, self.sort_period = float(dt), float(alpha), int(rule), int(sort_period)
         self.thermostat = bool(thermostat)
         self.ehat = self.xi = None
+        self.emb = None          # embedded beads (NEXT-1): dict(pos, vel, mass, chain_len, k, r0, nsub, cell)
         self.sigma = math.sqrt(self.kT / self.m)
         self.step_count = 0
         if init:
@@ -217,10 +246,27 @@ class OracleMPCD:
         self.tag = np.arange(self.N, dtype=np.uint32) if tag is None else np.ascontiguousarray(tag, dtype=np.uint32).copy()
         self.step_count = int(step)
 
+    def set_embedded(self, pos3, vel3, mass, chain_len, k, r0, md_substeps):
+        """NEXT-1 (BASELINE config 5): beads of linear harmonic chains that join the SRD collision and
+        move by md_substeps velocity-Verlet steps per collision step.  Beads are kept in double (A27)."""
+        assert self.rule == self.SRD and not self.thermostat
+        self.emb = dict(pos=np.ascontiguousarray(pos3, dtype=np.float64).copy(), vel=np.ascontiguousarray(vel3, dtype=np.float64).copy(),
+                        mass=np.ascontiguousarray(mass, dtype=np.float64).copy(), chain_len=int(chain_len), k=float(k), r0=float(r0),
+                        nsub=int(md_substeps), cell=None)
+
+    def _bin_embedded(self):
+        e = self.emb
+        p4 = np.zeros((e["pos"].shape[0], 4)); p4[:, :3] = e["pos"]
+        shift_used = self.shift.astype(self.dtype).astype(np.float64)        # the shift as the solvent's binning applies it (A5)
+        e["cell"] = bin_cells(p4, shift_used, self.a, self.n)
+
     # -- the blocks of Fig. 1 (PAPER.md:66-70) --
     def stream(self):
         assert float(np.abs(self.vel[:, :3]).max(initial=0.0)) * self.dt < min(self.L), "single-image wrap (A7)"
         stream(self.pos, self.vel, self.dt, self.L)
+        if self.emb is not None:     # the solute moves by MD over the same interval (PAPER.md:159)
+            e = self.emb
+            md_verlet(e["pos"], e["vel"], e["mass"], e["chain_len"], e["k"], e["r0"], self.L, self.dt / e["nsub"], e["nsub"])
 
     def shift_and_bin(self):
         t = self.step_count
@@ -232,6 +278,9 @@ class OracleMPCD:
         self.count, self.sumv, self.ke = reduce_cells(self.vel, self.cell, self.Nc, self.m)
         self.u, self.erel, self.kTc = finalize_cells(self.vel, self.cell, self.Nc, self.m, self.count, self.sumv)
         self.axis = draw_axis(self.seed, self.step_count, self.Nc)
+        if self.emb is not None:
+            self._bin_embedded()
+            self.u, self.Mc = embedded_means(self.m, self.count, self.sumv, self.emb["cell"], self.emb["vel"], self.emb["mass"])
         if self.thermostat:      # "we compute xi for each cell at the same time that we draw the rotation vectors"
             self.ehat, self.xi = thermostat_xi(self.seed, self.step_count, self.kT, self.count, self.erel)
 
@@ -242,6 +291,8 @@ class OracleMPCD:
 
     def collide_srd(self, alpha=None):
         alpha = self.alpha if alpha is None else alpha
+        if self.emb is not None:
+            collide_srd_beads(self.emb["vel"], self.emb["cell"], self.u, self.axis, alpha)
         if self.thermostat:
             collide_srd_xi(self.vel, self.cell, self.u, self.axis, self.xi, alpha)
         else:

@@ -46,3 +46,18 @@ def solvent(n, M, seed, *, a=1.0, kT=1.0, m=1.0, dtype=np.float32, N=None):
         vel4[lo:hi, :3] = (vel4[lo:hi, :3].astype(np.float64) - mean).astype(dtype)
     tag = np.arange(N, dtype=np.uint32)
     return pos4, vel4, tag
+
+
+def chains(n, n_chains, chain_len, seed, *, a=1.0, kT=1.0, mass=5.0, r0=0.5):
+    """Seeded beads of linear chains for BASELINE config 5: every chain is a random walk of step r0 from a uniform
+    random start (wrapped into the box), velocities N(0, kT/mass).  Returns (pos3, vel3, mass) as float64 arrays."""
+    rng = np.random.default_rng(seed)
+    L = np.array([int(x) for x in n], dtype=np.float64) * a
+    start = rng.random((n_chains, 1, 3)) * L
+    step = rng.standard_normal((n_chains, chain_len, 3))
+    step *= r0 / np.linalg.norm(step, axis=2, keepdims=True)
+    step[:, 0, :] = 0.0
+    pos = np.mod(start + np.cumsum(step, axis=1), L).reshape(-1, 3)
+    pos[pos >= L] = 0.0
+    vel = rng.standard_normal((n_chains * chain_len, 3)) * np.sqrt(kT / mass)
+    return np.ascontiguousarray(pos), np.ascontiguousarray(vel), np.full(n_chains * chain_len, float(mass))
