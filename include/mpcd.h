@@ -162,6 +162,20 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
 /* The shift used by the last bin, as applied (mixed mode: the fp32 value, A5).  s: host. */
 int mpcd_get_shift(mpcd_t *h, double s[3]);
 
+/* NEXT-1. Embedded solute (BASELINE config 5): nb beads of linear chains of chain_len beads each
+ * (nb a multiple of chain_len, chain_len <= 512), bead i of mass mass[i], consecutive beads of a chain joined by the
+ * harmonic bond U = k (r - r0)^2 / 2 (minimum image).  From then on the beads take part in the SRD collision -- the
+ * cell mean becomes (m sum_solvent v + sum_beads m_b v_b) / (m N_c + sum_beads m_b) and the beads are rotated about
+ * their cell's axis like the solvent -- and wherever the solvent streams over dt (mpcd_stream, mpcd_step) the beads
+ * are advanced by md_substeps velocity-Verlet steps of dt / md_substeps.  Beads are kept in double whatever the
+ * precision model (A27).  pos3, vel3: HOST, nb x 3 doubles, positions in [0, box); mass: HOST, nb doubles.  Needs the
+ * SRD rule without the cell thermostat (MPCD_EINVAL otherwise); the sort leaves the beads alone;
+ * mpcd_get_cells / mpcd_get_thermo report the solvent only.  Calling it again with the same nb replaces the state. */
+int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *vel3, const double *mass, int32_t chain_len, double k, double r0,
+                      int32_t md_substeps);
+/* Bead state to HOST buffers (any may be NULL): pos3, vel3 nb x 3 doubles, cell nb x i32 (last binning).  Synchronises. */
+int mpcd_get_embedded(mpcd_t *h, double *pos3, double *vel3, int32_t *cell);
+
 /* The thermostat's scale factor xi per cell for the current bin (opt.thermostat = 1; MPCD_ESTATE otherwise or when the
  * cell sums are not valid).  xi: host, Nc doubles.  Test accessor for the parity of PAPER.md:157. */
 int mpcd_get_xi(mpcd_t *h, double *xi);

@@ -50,7 +50,7 @@ EXPORTS = [
     "mpcd_default_options", "mpcd_create", "mpcd_create_ex", "mpcd_destroy", "mpcd_stream", "mpcd_shift_and_bin",
     "mpcd_collide_srd", "mpcd_collide_at", "mpcd_sort", "mpcd_step", "mpcd_get_state", "mpcd_set_state",
     "mpcd_get_cells", "mpcd_get_shift", "mpcd_get_thermo", "mpcd_get_stats", "mpcd_device_ptrs", "mpcd_last_error",
-    "mpcd_abi_version", "mpcd_build_info", "mpcd_test_philox", "mpcd_set_profiling", "mpcd_get_profile", "mpcd_get_xi",
+    "mpcd_abi_version", "mpcd_build_info", "mpcd_test_philox", "mpcd_set_profiling", "mpcd_get_profile", "mpcd_get_xi", "mpcd_set_embedded", "mpcd_get_embedded",
 ]
 PROF_KINDS = ("fused", "bin", "collide", "cells", "sort", "other", "fused_sort")
 
@@ -80,6 +80,8 @@ def load_library():
     lib.mpcd_get_cells.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.mpcd_get_shift.argtypes = [vp, P(dbl)]
     lib.mpcd_get_xi.argtypes = [vp, vp]
+    lib.mpcd_set_embedded.argtypes = [vp, i64, vp, vp, vp, i32, dbl, dbl, i32]
+    lib.mpcd_get_embedded.argtypes = [vp, vp, vp, vp]
     lib.mpcd_get_thermo.argtypes = [vp, P(dbl), P(dbl), P(dbl)]
     lib.mpcd_get_stats.argtypes = [vp, P(Stats)]
     lib.mpcd_device_ptrs.argtypes = [vp, P(vp), P(vp), P(vp), P(vp)]
@@ -232,6 +234,18 @@ class MPCD:
         if axis:
             o["axis"] = np.empty((Nc, 3))
         self._check(self.lib.mpcd_get_cells(self.h, _ptr(o["count"]), _ptr(o["sumv"]), _ptr(o["ke"]), _ptr(o["u"]), _ptr(o.get("axis")), _ptr(o["kTc"])))
+        return o
+
+    def set_embedded(self, pos3, vel3, mass, chain_len, k, r0, md_substeps):
+        pos3 = np.ascontiguousarray(pos3, dtype=np.float64); vel3 = np.ascontiguousarray(vel3, dtype=np.float64)
+        mass = np.ascontiguousarray(mass, dtype=np.float64)
+        assert pos3.shape == vel3.shape and pos3.shape[1] == 3 and mass.shape == (pos3.shape[0],)
+        self.nb = pos3.shape[0]
+        self._check(self.lib.mpcd_set_embedded(self.h, self.nb, _ptr(pos3), _ptr(vel3), _ptr(mass), int(chain_len), float(k), float(r0), int(md_substeps)))
+
+    def get_embedded(self):
+        o = dict(pos=np.empty((self.nb, 3)), vel=np.empty((self.nb, 3)), cell=np.empty(self.nb, np.int32))
+        self._check(self.lib.mpcd_get_embedded(self.h, _ptr(o["pos"]), _ptr(o["vel"]), _ptr(o["cell"])))
         return o
 
     def get_xi(self):

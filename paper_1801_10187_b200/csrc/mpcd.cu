@@ -42,6 +42,14 @@ struct mpcd {
     double *qacc[2] = {nullptr, nullptr};     // sum |v|^2 per cell
     double *at_acc[2] = {nullptr, nullptr};   // {Dx, Dy, Dz, -} per cell (AT only, allocated on first use)
     double *axis[2] = {nullptr, nullptr};     // {nx, ny, nz, -} per cell
+    // embedded solute (NEXT-1; mpcd_embedded.cuh): beads in double, their per-cell sums by step parity
+    int64_t emb_n = 0;
+    int32_t emb_chain_len = 0, emb_nsub = 0;
+    double emb_k = 0, emb_r0 = 0;
+    double4 *emb_pos = nullptr, *emb_vel = nullptr;
+    double *emb_acc[2] = {nullptr, nullptr};
+    bool emb_zeroed[2] = {false, false};
+    bool emb_binned = false;       // the beads are binned and summed for the current bin
     int32_t *cell_start = nullptr, *tile_sum = nullptr;
     int *d_max_occ = nullptr;
     double *d_scalars = nullptr;   // 8 doubles of scratch for reductions
@@ -178,6 +186,8 @@ template <typename T> PassArgs<T> make_args(mpcd_t *h, const PassPlan &pl)
     a.sums = h->acc[pl.cset];
     a.dsum = h->at_acc[pl.cset];
     a.axis = h->axis[pl.step_collide & 1];
+    a.esum = h->emb_acc[pl.cset];
+    a.mass = h->m;
     a.acc = h->acc[pl.bset];
     a.qacc = h->qacc[pl.bset];
     a.at_acc = h->at_acc[pl.bset];
@@ -229,6 +239,11 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
         CASE(kSRD | kStream | kBin | kEnergy | kSortOut)
         CASE(kATApply | kStream | kBin | kATDraw | kSortOut)
         CASE(kATApply | kStream | kBin | kATDraw | kEnergy | kSortOut)
+        CASE(kSRD | kEmbedded)
+        CASE(kSRD | kEmbedded | kStream | kBin)
+        CASE(kSRD | kEmbedded | kStream | kBin | kEnergy)
+        CASE(kSRD | kEmbedded | kStream | kBin | kSortOut)
+        CASE(kSRD | kEmbedded | kStream | kBin | kEnergy | kSortOut)
         CASE(kSRD | kThermo)
         CASE(kSRD | kThermo | kStream | kBin | kEnergy)
         CASE(kSRD | kThermo | kStream | kBin | kEnergy | kSortOut)
@@ -273,15 +288,18 @@ int prepare(mpcd_t *h, int zset, bool sums, bool at, bool want_axes, uint64_t ax
 {
     const bool zs = zset >= 0 && sums && !h->zeroed[zset];
     const bool za = zset >= 0 && at && h->at_acc[zset] && !h->at_zeroed[zset];
+    const bool ze = zset >= 0 && sums && h->emb_acc[zset] && !h->emb_zeroed[zset];      // the beads' sums go with the solvent's
     const int b = (int)(axis_step & 1);
     const bool ax = want_axes && !(h->axis_valid[b] && h->axis_step[b] == axis_step);
-    if (!zs && !za && !ax) return MPCD_OK;
+    if (!zs && !za && !ze && !ax) return MPCD_OK;
     ProfScope prof(h, MPCD_PROF_CELLS);
     cell_prepare<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(ax ? h->axis[b] : nullptr, h->seed, axis_step, zs ? h->acc[zset] : nullptr,
-                                                           zs ? h->qacc[zset] : nullptr, za ? h->at_acc[zset] : nullptr, h->Nc);
+                                                           zs ? h->qacc[zset] : nullptr, za ? h->at_acc[zset] : nullptr,
+                                                           ze ? h->emb_acc[zset] : nullptr, h->Nc);
     LAUNCH_CHECK(h);
     if (zs) h->zeroed[zset] = true;
     if (za) h->at_zeroed[zset] = true;
+    if (ze) h->emb_zeroed[zset] = true;
     if (ax) { h->axis_valid[b] = true; h->axis_step[b] = axis_step; h->xi_valid[b] = false; }
     return MPCD_OK;
 }
@@ -302,6 +320,54 @@ int thermostat(mpcd_t *h, uint64_t t)
     cell_thermostat<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[b], h->qacc[b], h->axis[b], h->Nc, h->m, h->kT, h->seed, t);
     LAUNCH_CHECK(h);
     h->xi_valid[b] = true;
+    return MPCD_OK;
+}
+
+// ---- embedded solute (NEXT-1) ----
+inline bool embedded(const mpcd_t *h) { return h->emb_n > 0; }
+
+EmbArgs emb_args(mpcd_t *h, int cset, int bset, uint64_t step_collide, const double shift[3], double alpha)
+{
+    EmbArgs e{};
+    e.pos = h->emb_pos; e.vel = h->emb_vel; e.nb = h->emb_n;
+    e.sums = h->acc[cset]; e.esum = h->emb_acc[cset]; e.axis = h->axis[step_collide & 1];
+    e.eacc = h->emb_acc[bset];
+    for (int d = 0; d < 3; ++d) { e.n[d] = h->n[d]; e.shift[d] = shift[d]; }
+    e.inv_a = 1.0 / h->a;
+    e.mass_solvent = h->m;
+    e.cos_a = std::cos(alpha); e.sin_a = std::sin(alpha);
+    return e;
+}
+
+// the beads' "streaming": md_substeps velocity-Verlet steps over one collision interval
+int emb_md(mpcd_t *h)
+{
+    MdArgs a{};
+    a.pos = h->emb_pos; a.vel = h->emb_vel; a.chain_len = h->emb_chain_len; a.nsub = h->emb_nsub;
+    a.k = h->emb_k; a.r0 = h->emb_r0; a.dt = h->opt.dt / h->emb_nsub;
+    for (int d = 0; d < 3; ++d) a.L[d] = h->box[d];
+    ProfScope prof(h, MPCD_PROF_OTHER);
+    emb_md_verlet<<<(unsigned)(h->emb_n / h->emb_chain_len), kEmbThreads, (size_t)h->emb_chain_len * 10 * sizeof(double), h->stream>>>(a);
+    LAUNCH_CHECK(h);
+    return MPCD_OK;
+}
+
+// bin the beads under `shift` and add them to the (zeroed) bead sums of set `bset`
+int emb_bin(mpcd_t *h, int bset, const double shift[3])
+{
+    ProfScope prof(h, MPCD_PROF_OTHER);
+    emb_bin_accumulate<<<grid_for(h->emb_n, kEmbThreads), kEmbThreads, 0, h->stream>>>(emb_args(h, bset, bset, 0, shift, 0.0));
+    LAUNCH_CHECK(h);
+    h->emb_zeroed[bset] = false;
+    return MPCD_OK;
+}
+
+int emb_rotate(mpcd_t *h, int cset, uint64_t step_collide, double alpha)
+{
+    const double zero[3] = {0, 0, 0};
+    ProfScope prof(h, MPCD_PROF_OTHER);
+    emb_collide<<<grid_for(h->emb_n, kEmbThreads), kEmbThreads, 0, h->stream>>>(emb_args(h, cset, cset, step_collide, zero, alpha));
+    LAUNCH_CHECK(h);
     return MPCD_OK;
 }
 
@@ -366,6 +432,7 @@ int bin_accumulate(mpcd_t *h, uint64_t t)
     h->bin_valid = true; h->bin_step = t;
     rc = ensure_axes(h, t);
     if (!rc && thermostatted(h)) rc = thermostat(h, t);
+    if (!rc && embedded(h)) { rc = emb_bin(h, set, pl.shift); h->emb_binned = rc == MPCD_OK; }
     if (rc) return rc;
     h->sums_valid = true; h->energy_valid = true; h->counts_valid = true;
     return MPCD_OK;
@@ -535,8 +602,9 @@ int mpcd_stream(mpcd_t *h)
     pl.cset = pl.bset = h->ccur;
     pl.step_collide = pl.step_bin = h->step;
     int rc = pass(h, kStream, pl);
+    if (!rc && embedded(h)) rc = emb_md(h);          // the solute moves by MD over the same interval
     if (rc) return rc;
-    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false;
+    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false; h->emb_binned = false;
     return MPCD_OK;
 }
 
@@ -558,9 +626,14 @@ int mpcd_collide_srd(mpcd_t *h, double alpha)
     pl.cset = pl.bset = h->ccur;
     pl.step_collide = pl.step_bin = h->step;
     pl.alpha = alpha;
-    rc = pass(h, kSRD | (thermostatted(h) ? kThermo : 0u), pl);
+    if (embedded(h)) {
+        if (!h->emb_binned) return fail(h, MPCD_ESTATE, "the embedded beads are not binned for this step: call mpcd_shift_and_bin%s");
+        rc = emb_rotate(h, h->ccur, h->step, alpha);
+        if (rc) return rc;
+    }
+    rc = pass(h, kSRD | (thermostatted(h) ? kThermo : 0u) | (embedded(h) ? kEmbedded : 0u), pl);
     if (rc) return rc;
-    h->sums_valid = false; h->energy_valid = false;
+    h->sums_valid = false; h->energy_valid = false; h->emb_binned = false;
     return MPCD_OK;
 }
 
@@ -569,6 +642,7 @@ int mpcd_collide_at(mpcd_t *h)
     if (!h) return MPCD_EINVAL;
     if (!(h->bin_valid && h->bin_step == h->step && h->sums_valid))
         return fail(h, MPCD_ESTATE, "collide_at needs mpcd_shift_and_bin for the current step first%s");
+    if (embedded(h)) return fail(h, MPCD_ESTATE, "embedded beads take part in the SRD rule only%s");
     int rc = ensure_at_buffers(h);
     if (rc) return rc;
     const int set = h->ccur;
@@ -599,6 +673,9 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     if (nsteps < 0) return fail(h, MPCD_EINVAL, "nsteps must be >= 0%s");
     if (nsteps == 0) return MPCD_OK;
     const bool at = h->opt.rule == MPCD_AT;
+    const bool emb = embedded(h);
+    if (emb && at) return fail(h, MPCD_ESTATE, "embedded beads take part in the SRD rule only%s");
+    const unsigned fb = emb ? kEmbedded : 0u;
     const unsigned ft = (!at && thermostatted(h)) ? kThermo : 0u;
     const unsigned fe = (h->opt.cell_energy != 0 || ft) ? kEnergy : 0u;      // the thermostat needs the cell energies
     int rc = at ? ensure_at_buffers(h) : MPCD_OK;
@@ -615,6 +692,8 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     pl.step_collide = pl.step_bin = t;
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
     rc = pass(h, kStream | kBin | fe | (at ? (kATDraw | kATStored) : 0u), pl);   // AT: vel.xyz carries dv between the launches of this call
+    if (!rc && emb) rc = emb_md(h);
+    if (!rc && emb) rc = emb_bin(h, set, pl.shift);
     if (rc) return rc;
     if (ft) { rc = thermostat(h, t); if (rc) return rc; }
     bool sort_pending = sort_due(h, t);            // sort by the cells of step t: done by the next fused kernel on its way out
@@ -625,11 +704,17 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
         rc = prepare(h, nxt, true, at, !at, t + 1);
         if (rc) return rc;
         if (sort_pending) { rc = scan_counts(h, set); if (rc) return rc; }
+        if (emb) {                                  // beads: collide(t) with the complete sums of step t, then MD over the next interval
+            rc = emb_rotate(h, set, t, h->opt.alpha);
+            if (!rc) rc = emb_md(h);
+            if (rc) return rc;
+        }
         shift_for(h, t + 1, pl.shift);
+        if (emb) { rc = emb_bin(h, nxt, pl.shift); if (rc) return rc; }
         pl.cset = set; pl.bset = nxt;
         pl.step_collide = t; pl.step_bin = t + 1;
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
-        rc = pass(h, (at ? (kATApply | kATDraw | kATStored) : (kSRD | ft)) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
+        rc = pass(h, (at ? (kATApply | kATDraw | kATStored) : (kSRD | ft | fb)) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
         if (rc) return rc;
         if (sort_pending) { h->pcur ^= 1; h->sorts += 1; }
         set = nxt; t += 1;
@@ -640,8 +725,10 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     // last collision
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;
-    rc = pass(h, at ? (kATApply | kATStored) : (kSRD | ft), pl);
+    if (emb) { rc = emb_rotate(h, set, t, h->opt.alpha); if (rc) return rc; }
+    rc = pass(h, at ? (kATApply | kATStored) : (kSRD | ft | fb), pl);
     if (rc) return rc;
+    h->emb_binned = false;
     h->ccur = set;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = pl.shift[d];
     h->bin_valid = true; h->bin_step = t; h->counts_valid = true;
@@ -715,6 +802,53 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
     if (cudaStreamSynchronize(h->stream) != cudaSuccess && rc == MPCD_OK) rc = fail(h, MPCD_ECUDA, "get_cells sync failed%s");
     cudaFree(tmp);
     return rc;
+}
+
+int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *vel3, const double *mass, int32_t chain_len, double k, double r0,
+                      int32_t md_substeps)
+{
+    if (!h) return MPCD_EINVAL;
+    if (h->opt.rule != MPCD_SRD || thermostatted(h)) return fail(h, MPCD_EINVAL, "embedded beads need the SRD rule without the cell thermostat%s");
+    if (nb < 1 || !pos3 || !vel3 || !mass || chain_len < 1 || chain_len > kMaxChainLen || nb % chain_len != 0 || !(k >= 0) || !(r0 >= 0) || md_substeps < 1)
+        return fail(h, MPCD_EINVAL, "set_embedded: nb >= 1 a multiple of chain_len in [1, 512], k, r0 >= 0, md_substeps >= 1%s");
+    std::vector<double4> hp((size_t)nb), hv((size_t)nb);
+    for (int64_t i = 0; i < nb; ++i) {
+        if (!(mass[i] > 0)) return fail(h, MPCD_EINVAL, "set_embedded: masses must be positive%s");
+        for (int d = 0; d < 3; ++d)
+            if (!(pos3[3 * i + d] >= 0.0 && pos3[3 * i + d] < h->box[d])) return fail(h, MPCD_EINVAL, "set_embedded: positions must lie in [0, box)%s");
+        hp[i] = double4{pos3[3 * i], pos3[3 * i + 1], pos3[3 * i + 2], mass[i]};
+        hv[i] = double4{vel3[3 * i], vel3[3 * i + 1], vel3[3 * i + 2], 0.0};
+    }
+    if (h->emb_n != nb) {
+        if (h->emb_n != 0) return fail(h, MPCD_EINVAL, "set_embedded: the number of beads of a handle cannot change%s");
+        int rc = dev_alloc_t(h, &h->emb_pos, (size_t)nb);
+        if (!rc) rc = dev_alloc_t(h, &h->emb_vel, (size_t)nb);
+        for (int s = 0; s < 2 && !rc; ++s) { rc = dev_alloc_t(h, &h->emb_acc[s], (size_t)h->Nc * 4); h->emb_zeroed[s] = false; }
+        if (rc) return rc;
+    }
+    CUDA_TRY(h, cudaMemcpyAsync(h->emb_pos, hp.data(), (size_t)nb * sizeof(double4), cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(h->emb_vel, hv.data(), (size_t)nb * sizeof(double4), cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    h->emb_n = nb; h->emb_chain_len = chain_len; h->emb_nsub = md_substeps; h->emb_k = k; h->emb_r0 = r0;
+    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false; h->emb_binned = false;
+    return MPCD_OK;
+}
+
+int mpcd_get_embedded(mpcd_t *h, double *pos3, double *vel3, int32_t *cell)
+{
+    if (!h) return MPCD_EINVAL;
+    if (!embedded(h)) return fail(h, MPCD_ESTATE, "no embedded beads%s");
+    const size_t nb = (size_t)h->emb_n;
+    std::vector<double4> hp(nb), hv(nb);
+    CUDA_TRY(h, cudaMemcpyAsync(hp.data(), h->emb_pos, nb * sizeof(double4), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(hv.data(), h->emb_vel, nb * sizeof(double4), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    for (size_t i = 0; i < nb; ++i) {
+        if (pos3) { pos3[3 * i] = hp[i].x; pos3[3 * i + 1] = hp[i].y; pos3[3 * i + 2] = hp[i].z; }
+        if (vel3) { vel3[3 * i] = hv[i].x; vel3[3 * i + 1] = hv[i].y; vel3[3 * i + 2] = hv[i].z; }
+        if (cell) { long long c; std::memcpy(&c, &hv[i].w, sizeof(c)); cell[i] = (int32_t)c; }
+    }
+    return MPCD_OK;
 }
 
 int mpcd_get_xi(mpcd_t *h, double *xi)

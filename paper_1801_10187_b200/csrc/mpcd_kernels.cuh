@@ -15,6 +15,8 @@
 //   kATStored a7     inside mpcd_step: kATDraw leaves the drawn dv in vel.xyz instead of the velocity (the AT update
 //                    v = u + dv - D/N_c does not depend on the old velocity, which has been summed by then), and the
 //                    next kATApply takes it from there instead of regenerating it: one Gaussian draw per particle-step
+//   kEmbedded a5     with kSRD: the cell mean is mass-weighted over the solvent sums and the embedded beads' sums
+//                    (mpcd_embedded.cuh)
 //   kSortOut  a8     sort by cell on the way out: instead of in place, the particle is written
 //                    to slot cell_start[c] + (atomic cursor) of the duplicate arrays, c = its cell in the step
 //                    being collided; the separate read-and-scatter pass of the sort disappears
@@ -26,10 +28,11 @@
 // of the next step and a zeroed accumulator set.
 #pragma once
 #include "mpcd_device.cuh"
+#include "mpcd_embedded.cuh"
 
 namespace mpcdk {
 
-enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u };
+enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u, kEmbedded = 512u };
 
 template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
@@ -38,7 +41,9 @@ template <typename T> struct PassArgs {
     // cell arrays of the step being collided (read only)
     const double *sums;   // {Sx, Sy, Sz, N} per cell
     const double *dsum;   // {Dx, Dy, Dz, -} per cell: sum of the thermostat draws (AT)
-    const double *axis;   // {nx, ny, nz, -} per cell (SRD)
+    const double *axis;   // {nx, ny, nz, xi} per cell (SRD; xi = thermostat factor)
+    const double *esum;   // {sum m v, sum m} of the embedded beads per cell (kEmbedded)
+    double mass;          // solvent particle mass (kEmbedded)
     // accumulators of the step being binned
     double *acc;          // {Sx, Sy, Sz, N} per cell
     double *qacc;         // sum |v|^2 per cell (kEnergy)
@@ -116,8 +121,13 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
         if (valid) {
             const f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);    // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
             const f64x4 n = ld256_nc(a.axis + 4 * (size_t)c);
-            const double inv = __drcp_rn(s.w);                   // N_c >= 1: this particle is a member
-            const double ux = s.x * inv, uy = s.y * inv, uz = s.z * inv;
+            double ux, uy, uz;
+            if (F & kEmbedded) {
+                embedded_mean(s, ld256_nc(a.esum + 4 * (size_t)c), a.mass, ux, uy, uz);
+            } else {
+                const double inv = __drcp_rn(s.w);               // N_c >= 1: this particle is a member
+                ux = s.x * inv; uy = s.y * inv; uz = s.z * inv;
+            }
             const double wx = (double)v.x - ux, wy = (double)v.y - uy, wz = (double)v.z - uz;   // lines 5-6
             const double ndw = n.x * wx + n.y * wy + n.z * wz;                                  // line 7
             const double omc = 1.0 - a.cos_a;
@@ -192,13 +202,15 @@ __global__ void __launch_bounds__(256) cells_of_particles(const PassArgs<T> a, i
 // accumulator set.  Any pointer may be NULL.  One launch per step in mpcd_step: the axes of step t + 1
 // together with the zeroing of the set of step t + 2.
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) cell_prepare(double *axis, uint64_t seed, uint64_t step, double *zero_acc, double *zero_q, double *zero_at, int64_t Nc)
+__global__ void __launch_bounds__(256) cell_prepare(double *axis, uint64_t seed, uint64_t step, double *zero_acc, double *zero_q, double *zero_at, double *zero_emb,
+                                                    int64_t Nc)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
     if (zero_acc) st256(zero_acc + 4 * c, 0.0, 0.0, 0.0, 0.0);
     if (zero_q) zero_q[c] = 0.0;
     if (zero_at) st256(zero_at + 4 * c, 0.0, 0.0, 0.0, 0.0);
+    if (zero_emb) st256(zero_emb + 4 * c, 0.0, 0.0, 0.0, 0.0);
     if (axis) {
         double nx, ny, nz;
         draw_axis(seed, step, (uint32_t)c, nx, ny, nz);

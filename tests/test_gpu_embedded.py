@@ -1,0 +1,104 @@
+"""GPU parity for the embedded solute (BASELINE config 5) through the C ABI:
+MD of the beads, mass-weighted cell means, the collision of beads and solvent against the oracle, and the invariants
+of a config-5-like run (total momentum, bond lengths, equipartition)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1801_10187_b200 import synth
+
+pytestmark = pytest.mark.gpu
+K, R0, NSUB, MB = 1000.0, 0.5, 10, 5.0
+
+
+def _pair(oracle, n, M, seed, dtype, n_chains, chain_len, **kw):
+    from paper_1801_10187_b200 import MPCD
+    pos, vel, tag = synth.solvent(n, M, seed=seed, dtype=dtype)
+    bp, bv, bm = synth.chains(n, n_chains, chain_len, seed=seed + 1, mass=MB, r0=R0)
+    box = [float(x) for x in n]
+    g = MPCD(box, pos.shape[0], seed=seed, precision="fp64" if dtype == np.float64 else "mixed", init_state=False, **kw)
+    g.set_state(pos, vel, tag); g.set_embedded(bp, bv, bm, chain_len, K, R0, NSUB)
+    o = oracle.OracleMPCD(box, pos.shape[0], seed=seed, dtype=dtype, init=False, **kw)
+    o.set_state(pos, vel, tag); o.set_embedded(bp, bv, bm, chain_len, K, R0, NSUB)
+    return g, o, bm
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_md_bin_and_collision_with_beads_match_the_oracle(oracle, dtype):
+    g, o, bm = _pair(oracle, (9, 8, 7), 5, 40, dtype, 14, 12)
+    for _ in range(2):
+        g.stream(); o.stream()
+        e = g.get_embedded()
+        np.testing.assert_allclose(e["pos"], o.emb["pos"], rtol=0, atol=1e-12)      # velocity Verlet, 10 substeps
+        np.testing.assert_allclose(e["vel"], o.emb["vel"], rtol=0, atol=1e-11)
+        g.shift_and_bin(); o.shift_and_bin()
+        assert np.array_equal(g.get_embedded()["cell"], o.emb["cell"])              # bead cells bit-exact
+        assert np.array_equal(g.get_state()["cell"], o.cell)
+        g.collide_srd(math.radians(130.0)); o.collide_srd(math.radians(130.0))
+        np.testing.assert_allclose(g.get_embedded()["vel"], o.emb["vel"], rtol=0, atol=1e-11)
+        err = np.max(np.abs(g.get_state()["vel"][:, :3].astype(np.float64) - o.vel[:, :3].astype(np.float64)))
+        assert err <= (1e-12 if dtype == np.float64 else 1e-5), err
+        st = g.get_state()                                                          # teacher-force the next round
+        o.set_state(st["pos"], st["vel"], st["tag"], step=st["step"] + 1)
+        g.set_state(st["pos"], st["vel"], st["tag"], step=st["step"] + 1)
+        e = g.get_embedded(); o.emb["pos"][:] = e["pos"]; o.emb["vel"][:] = e["vel"]
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_fused_steps_with_beads_match_the_oracle(oracle, dtype):
+    g, o, bm = _pair(oracle, (10, 9, 8), 5, 41, dtype, 10, 20, sort_period=2)
+    g.step(3); o.step(3)
+    s = g.get_state(); e = g.get_embedded()
+    a, b = np.argsort(s["tag"]), np.argsort(o.tag)
+    tol = 1e-11 if dtype == np.float64 else 3e-5
+    assert np.max(np.abs(s["vel"][a][:, :3].astype(np.float64) - o.vel[b][:, :3].astype(np.float64))) <= tol
+    assert np.max(np.abs(e["vel"] - o.emb["vel"])) <= tol
+    assert np.max(np.abs(e["pos"] - o.emb["pos"])) <= tol
+    assert np.array_equal(e["cell"], o.emb["cell"])
+
+
+def test_config5_like_run_conserves_momentum_and_equilibrates():
+    """BASELINE config 5 at reduced size: 32^3 cells, density 5, 100 chains of 50 beads (mass 5, k = 1000, r0 = 0.5),
+    10 MD substeps per collision, mixed precision; the beads start twice too hot."""
+    from paper_1801_10187_b200 import MPCD
+    n, M = (32, 32, 32), 5
+    pos, vel, tag = synth.solvent(n, M, seed=50, dtype=np.float32)
+    bp, bv, bm = synth.chains(n, 100, 50, seed=51, kT=2.0, mass=MB, r0=R0)
+    N = pos.shape[0]
+    g = MPCD([float(x) for x in n], N, seed=50, init_state=False)
+    g.set_state(pos, vel, tag); g.set_embedded(bp, bv, bm, 50, K, R0, NSUB)
+    P0 = vel[:, :3].astype(np.float64).sum(axis=0) + (bm[:, None] * bv).sum(axis=0)
+    g.step(200)
+    kTb = []
+    for _ in range(20):
+        g.step(10)
+        kTb.append((bm[:, None] * g.get_embedded()["vel"] ** 2).sum() / (3 * bm.size))
+    s = g.get_state(); e = g.get_embedded()
+    P1 = s["vel"][:, :3].astype(np.float64).sum(axis=0) + (bm[:, None] * e["vel"]).sum(axis=0)
+    assert np.max(np.abs(P1 - P0)) / (N + MB * bm.size) <= 1e-6                     # total momentum incl. the beads
+    assert abs(np.mean(kTb) - 1.0) < 0.05, np.mean(kTb)                            # equipartition with the solvent at kT = 1
+    d = e["pos"].reshape(100, 50, 3); bond = d[:, 1:] - d[:, :-1]; bond -= 32.0 * np.round(bond / 32.0)
+    r = np.linalg.norm(bond, axis=2)
+    assert abs(r.mean() - R0) < 0.02 and abs(r.std() - math.sqrt(1.0 / K)) < 0.01   # thermal bond fluctuations sqrt(kT/k)
+    assert g.stats()["sorts"] == 16 and np.array_equal(np.sort(s["tag"]), tag)
+    g.close()
+
+
+def test_embedded_argument_checks():
+    from paper_1801_10187_b200 import MPCD, MPCDError
+    bp, bv, bm = synth.chains((4, 4, 4), 2, 5, seed=1)
+    for kw in (dict(rule="at"), dict(thermostat=True)):
+        g = MPCD([4.0] * 3, 320, seed=1, **kw)
+        with pytest.raises(MPCDError) as err:
+            g.set_embedded(bp, bv, bm, 5, K, R0, NSUB)
+        assert err.value.code == -1
+        g.close()
+    g = MPCD([4.0] * 3, 320, seed=1)
+    for bad in (dict(chain_len=3), dict(md_substeps=0), dict(chain_len=1024)):
+        args = dict(chain_len=5, k=K, r0=R0, md_substeps=NSUB); args.update(bad)
+        with pytest.raises(MPCDError):
+            g.set_embedded(bp, bv, bm, **args)
+    with pytest.raises(MPCDError):
+        g.get_embedded()
+    g.close()
