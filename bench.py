@@ -132,6 +132,11 @@ def oracle_sample(cfg, precision, steps, warmup, n_sample):
     o = O.OracleMPCD([float(x) for x in n_sample], pos.shape[0], seed=cfg["seed"], dtype=dtype, init=False,
                      rule=1 if cfg["rule"] == "at" else 0, sort_period=25)
     o.set_state(pos, vel, tag)
+    if "chains" in cfg:      # the same bead : solvent ratio in the sample box
+        ch = cfg["chains"]
+        nch = max(1, round(ch["n_chains"] * pos.shape[0] / (cfg["n"][0] * cfg["n"][1] * cfg["n"][2] * cfg["M"])))
+        bp, bv, bm = synth.chains(n_sample, nch, ch["chain_len"], seed=cfg["seed"] + 1, mass=ch["mass"], r0=ch["r0"])
+        o.set_embedded(bp, bv, bm, ch["chain_len"], ch["k"], ch["r0"], ch["md_substeps"])
     for _ in range(warmup):
         o.step()
     t0 = time.perf_counter()
@@ -169,7 +174,12 @@ def run_reference(args, cfg, rank, world):
 
 def workload_config(args, cfg):
     n = cfg["n"]
-    return {"workload": f"{args.config}: pure MPCD-{cfg['rule'].upper()} solvent, {n[0]}x{n[1]}x{n[2]} cells (a=1), density {cfg['M']}, "
+    solute = ""
+    if "chains" in cfg:
+        ch = cfg["chains"]
+        solute = (f" + {ch['n_chains']} chains of {ch['chain_len']} beads (mass {ch['mass']:g}, harmonic bonds k={ch['k']:g}, r0={ch['r0']:g}, "
+                  f"{ch['md_substeps']} velocity-Verlet substeps per collision) joining the collisions")
+    return {"workload": f"{args.config}: MPCD-{cfg['rule'].upper()} solvent{solute}, {n[0]}x{n[1]}x{n[2]} cells (a=1), density {cfg['M']}, "
                         f"{n[0] * n[1] * n[2] * cfg['M']} particles, alpha=130deg, dt=0.1, random grid shift, sort every 25, {args.precision} precision",
             "particles_per_gpu": n[0] * n[1] * n[2] * cfg["M"], "cells_per_gpu": n[0] * n[1] * n[2],
             "precision": args.precision, "cell_energy": bool(args.cell_energy),
@@ -227,6 +237,10 @@ def main():
     sim = MPCD([float(x) for x in n], N, seed=seed, precision=args.precision, rule=cfg["rule"], sort_period=args.sort_period,
                cell_energy=bool(args.cell_energy), init_state=False, device=f"cuda:{local_rank}")
     sim.set_state(pos, vel, tag)
+    if "chains" in cfg:
+        ch = cfg["chains"]
+        bp, bv, bm = synth.chains(n, ch["n_chains"], ch["chain_len"], seed=seed + 1, mass=ch["mass"], r0=ch["r0"])
+        sim.set_embedded(bp, bv, bm, ch["chain_len"], ch["k"], ch["r0"], ch["md_substeps"])
 
     # ---- device-resident throughput ----
     sim.step(args.warmup)

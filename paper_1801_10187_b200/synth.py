@@ -16,6 +16,9 @@ CONFIGS = {
     "C2": dict(n=(64, 64, 64), M=10, seed=10187, rule="srd", steps=1000),
     "C3": dict(n=(200, 200, 200), M=10, seed=180110187, rule="srd", steps=500),
     "C4": dict(n=(256, 256, 128), M=5, seed=42, rule="at", steps=500),
+    # polymer solution: + 1000 chains of 50 beads (mass 5, harmonic bonds k = 1000, r0 = 0.5), 10 MD substeps per collision
+    "C5": dict(n=(100, 100, 100), M=5, seed=5, rule="srd", steps=500,
+               chains=dict(n_chains=1000, chain_len=50, mass=5.0, k=1000.0, r0=0.5, md_substeps=10)),
 }
 
 
