@@ -118,7 +118,12 @@ int dev_alloc(mpcd_t *h, void **out, size_t bytes)
         cudaError_t e = cudaMalloc(&p, bytes);
         if (e != cudaSuccess) { cudaGetLastError(); return fail(h, MPCD_ENOMEM, "cudaMalloc: %s", cudaGetErrorString(e)); }
     }
-    h->buffers.push_back(Buffer{p, bytes});
+    try {
+        h->buffers.push_back(Buffer{p, bytes});
+    } catch (...) {
+        if (h->opt.free_fn) h->opt.free_fn(p, h->opt.alloc_user); else if (!h->opt.alloc_fn) cudaFree(p);
+        return fail(h, MPCD_ENOMEM, "host bookkeeping allocation failed%s");
+    }
     h->device_bytes += bytes;
     *out = p;
     return MPCD_OK;
@@ -141,7 +146,7 @@ struct ProfScope {   // brackets the launches of one kind with a CUDA event pair
     {
         if (!a) return;
         cudaEventRecord(b, h->stream);
-        h->timed.push_back(mpcd::Timed{a, b, kind});
+        try { h->timed.push_back(mpcd::Timed{a, b, kind}); } catch (...) { cudaEventDestroy(a); cudaEventDestroy(b); }
     }
 };
 
@@ -811,7 +816,8 @@ int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *v
     if (h->opt.rule != MPCD_SRD || thermostatted(h)) return fail(h, MPCD_EINVAL, "embedded beads need the SRD rule without the cell thermostat%s");
     if (nb < 1 || !pos3 || !vel3 || !mass || chain_len < 1 || chain_len > kMaxChainLen || nb % chain_len != 0 || !(k >= 0) || !(r0 >= 0) || md_substeps < 1)
         return fail(h, MPCD_EINVAL, "set_embedded: nb >= 1 a multiple of chain_len in [1, 512], k, r0 >= 0, md_substeps >= 1%s");
-    std::vector<double4> hp((size_t)nb), hv((size_t)nb);
+    std::vector<double4> hp, hv;
+    try { hp.resize((size_t)nb); hv.resize((size_t)nb); } catch (...) { return fail(h, MPCD_ENOMEM, "set_embedded: host staging allocation failed%s"); }
     for (int64_t i = 0; i < nb; ++i) {
         if (!(mass[i] > 0)) return fail(h, MPCD_EINVAL, "set_embedded: masses must be positive%s");
         for (int d = 0; d < 3; ++d)
@@ -839,7 +845,8 @@ int mpcd_get_embedded(mpcd_t *h, double *pos3, double *vel3, int32_t *cell)
     if (!h) return MPCD_EINVAL;
     if (!embedded(h)) return fail(h, MPCD_ESTATE, "no embedded beads%s");
     const size_t nb = (size_t)h->emb_n;
-    std::vector<double4> hp(nb), hv(nb);
+    std::vector<double4> hp, hv;
+    try { hp.resize(nb); hv.resize(nb); } catch (...) { return fail(h, MPCD_ENOMEM, "get_embedded: host staging allocation failed%s"); }
     CUDA_TRY(h, cudaMemcpyAsync(hp.data(), h->emb_pos, nb * sizeof(double4), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaMemcpyAsync(hv.data(), h->emb_vel, nb * sizeof(double4), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
