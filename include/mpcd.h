@@ -39,7 +39,7 @@
 extern "C" {
 #endif
 
-#define MPCD_ABI_VERSION 1
+#define MPCD_ABI_VERSION 2
 
 /* status codes */
 #define MPCD_OK      0
@@ -79,6 +79,11 @@ typedef struct mpcd_options {
     int32_t thermostat;    /* 1: Maxwell-Boltzmann cell thermostat for the SRD rule (PAPER.md:45-50 eq. 3, :157): the relative
                               velocities of every cell with N_c >= 2 are scaled by xi = sqrt(E^/E_k), E^ ~ Gamma(3 (N_c - 1) / 2, kT);
                               default 0.  Ignored by the AT rule, which is isothermal by construction */
+    int32_t deterministic; /* 1: deterministic accumulation (NEXT-3; PAPER.md:124-126 names the alternative): the cell sums are 64-bit
+                              fixed-point integers (40 fractional bits), so the trajectory is bit-reproducible whatever the order of
+                              warps, atomics and particles in memory; results stay within the mixed-model tolerance of the fp64
+                              sums.  Mixed model + SRD rule only (MPCD_EINVAL otherwise; no embedded beads); default 0 */
+    int32_t reserved1;
     void *stream;          /* cudaStream_t the library enqueues on; NULL = the legacy default stream */
     mpcd_alloc_fn alloc_fn;
     mpcd_free_fn free_fn;

@@ -28,6 +28,7 @@ class Options(C.Structure):
     _fields_ = [
         ("precision", C.c_int32), ("rule", C.c_int32), ("dt", C.c_double), ("alpha", C.c_double),
         ("sort_period", C.c_int32), ("cell_energy", C.c_int32), ("init_state", C.c_int32), ("thermostat", C.c_int32),
+        ("deterministic", C.c_int32), ("reserved1", C.c_int32),
         ("stream", C.c_void_p), ("alloc_fn", ALLOC_FN), ("free_fn", FREE_FN), ("alloc_user", C.c_void_p),
     ]
 
@@ -138,7 +139,7 @@ class MPCD:
     """One MPCD solvent on one GPU.  Method names are the C ABI's without the prefix."""
 
     def __init__(self, box, N, a=1.0, m=1.0, kT=1.0, seed=0, *, precision="mixed", rule="srd", dt=0.1,
-                 alpha=math.radians(130.0), sort_period=25, cell_energy=True, init_state=True, thermostat=False,
+                 alpha=math.radians(130.0), sort_period=25, cell_energy=True, init_state=True, thermostat=False, deterministic=False,
                  device="cuda:0", use_torch_allocator=True, stream=None):
         import torch
         if not torch.cuda.is_available():
@@ -156,6 +157,7 @@ class MPCD:
         opt.dt, opt.alpha = float(dt), float(alpha)
         opt.sort_period, opt.cell_energy, opt.init_state = int(sort_period), int(bool(cell_energy)), int(bool(init_state))
         opt.thermostat = int(bool(thermostat))
+        opt.deterministic = int(bool(deterministic))
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         opt.stream = C.c_void_p(self._stream.cuda_stream)
         self._alloc = TorchAllocator(device) if use_torch_allocator else None

@@ -249,6 +249,17 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
         CASE(kSRD | kEmbedded | kStream | kBin | kEnergy)
         CASE(kSRD | kEmbedded | kStream | kBin | kSortOut)
         CASE(kSRD | kEmbedded | kStream | kBin | kEnergy | kSortOut)
+        CASE(kBin | kEnergy | kFixed)
+        CASE(kStream | kBin | kFixed)
+        CASE(kStream | kBin | kEnergy | kFixed)
+        CASE(kSRD | kFixed)
+        CASE(kSRD | kStream | kBin | kFixed)
+        CASE(kSRD | kStream | kBin | kEnergy | kFixed)
+        CASE(kSRD | kStream | kBin | kSortOut | kFixed)
+        CASE(kSRD | kStream | kBin | kEnergy | kSortOut | kFixed)
+        CASE(kSRD | kThermo | kFixed)
+        CASE(kSRD | kThermo | kStream | kBin | kEnergy | kFixed)
+        CASE(kSRD | kThermo | kStream | kBin | kEnergy | kSortOut | kFixed)
         CASE(kSRD | kThermo)
         CASE(kSRD | kThermo | kStream | kBin | kEnergy)
         CASE(kSRD | kThermo | kStream | kBin | kEnergy | kSortOut)
@@ -312,6 +323,8 @@ inline int zero_set(mpcd_t *h, int s, bool sums, bool at) { return prepare(h, s,
 inline int ensure_axes(mpcd_t *h, uint64_t t) { return prepare(h, -1, false, false, true, t); }
 
 inline bool thermostatted(const mpcd_t *h) { return h->opt.thermostat != 0; }
+inline bool deterministic(const mpcd_t *h) { return h->opt.deterministic != 0; }
+inline unsigned fixed_flag(const mpcd_t *h) { return h->opt.deterministic != 0 ? kFixed : 0u; }
 
 // Maxwell-Boltzmann cell thermostat: xi of every cell from the complete sums (incl. energy) of step t in
 // set t & 1, into the 4th word of that step's axis sectors.
@@ -322,7 +335,7 @@ int thermostat(mpcd_t *h, uint64_t t)
     int rc = ensure_axes(h, t);
     if (rc) return rc;
     ProfScope prof(h, MPCD_PROF_CELLS);
-    cell_thermostat<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[b], h->qacc[b], h->axis[b], h->Nc, h->m, h->kT, h->seed, t);
+    cell_thermostat<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[b], h->qacc[b], h->axis[b], h->Nc, h->m, h->kT, h->seed, t, deterministic(h));
     LAUNCH_CHECK(h);
     h->xi_valid[b] = true;
     return MPCD_OK;
@@ -381,11 +394,11 @@ int scan_counts(mpcd_t *h, int s)
 {
     const int ntiles = (int)((h->Nc + kScanTile - 1) / kScanTile);
     ProfScope prof(h, MPCD_PROF_SORT);
-    scan_tile_sums<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum);
+    scan_tile_sums<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum, deterministic(h));
     LAUNCH_CHECK(h);
     scan_tile_offsets<<<1, 1024, 0, h->stream>>>(h->tile_sum, ntiles);
     LAUNCH_CHECK(h);
-    scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum, h->cell_start);
+    scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum, h->cell_start, deterministic(h));
     LAUNCH_CHECK(h);
     return MPCD_OK;
 }
@@ -430,7 +443,7 @@ int bin_accumulate(mpcd_t *h, uint64_t t)
     int rc = zero_set(h, set, true, false);
     if (rc) return rc;
     h->zeroed[set] = false;
-    rc = pass(h, kBin | kEnergy, pl);
+    rc = pass(h, kBin | kEnergy | fixed_flag(h), pl);
     if (rc) return rc;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = pl.shift[d];
     h->ccur = set;
@@ -533,6 +546,8 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
     if (o.precision != MPCD_MIXED && o.precision != MPCD_FP64) return fail(nullptr, MPCD_EINVAL, "bad precision%s");
     if (o.rule != MPCD_SRD && o.rule != MPCD_AT) return fail(nullptr, MPCD_EINVAL, "bad rule%s");
     if (o.thermostat != 0 && o.thermostat != 1) return fail(nullptr, MPCD_EINVAL, "thermostat must be 0 or 1%s");
+    if (o.deterministic != 0 && (o.deterministic != 1 || o.precision != MPCD_MIXED || o.rule != MPCD_SRD))
+        return fail(nullptr, MPCD_EINVAL, "deterministic accumulation is 0 or 1 and needs the mixed model and the SRD rule%s");
     if (!(o.dt > 0) || o.sort_period < 0) return fail(nullptr, MPCD_EINVAL, "dt must be > 0 and sort_period >= 0%s");
     if ((o.alloc_fn == nullptr) != (o.free_fn == nullptr)) return fail(nullptr, MPCD_EINVAL, "alloc_fn and free_fn must be given together%s");
     int32_t n[3];
@@ -636,7 +651,7 @@ int mpcd_collide_srd(mpcd_t *h, double alpha)
         rc = emb_rotate(h, h->ccur, h->step, alpha);
         if (rc) return rc;
     }
-    rc = pass(h, kSRD | (thermostatted(h) ? kThermo : 0u) | (embedded(h) ? kEmbedded : 0u), pl);
+    rc = pass(h, kSRD | (thermostatted(h) ? kThermo : 0u) | (embedded(h) ? kEmbedded : 0u) | fixed_flag(h), pl);
     if (rc) return rc;
     h->sums_valid = false; h->energy_valid = false; h->emb_binned = false;
     return MPCD_OK;
@@ -680,7 +695,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     const bool at = h->opt.rule == MPCD_AT;
     const bool emb = embedded(h);
     if (emb && at) return fail(h, MPCD_ESTATE, "embedded beads take part in the SRD rule only%s");
-    const unsigned fb = emb ? kEmbedded : 0u;
+    const unsigned fb = (emb ? kEmbedded : 0u) | fixed_flag(h);    // flags of the SRD gather; kFixed also goes with every kBin
     const unsigned ft = (!at && thermostatted(h)) ? kThermo : 0u;
     const unsigned fe = (h->opt.cell_energy != 0 || ft) ? kEnergy : 0u;      // the thermostat needs the cell energies
     int rc = at ? ensure_at_buffers(h) : MPCD_OK;
@@ -696,7 +711,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
-    rc = pass(h, kStream | kBin | fe | (at ? (kATDraw | kATStored) : 0u), pl);   // AT: vel.xyz carries dv between the launches of this call
+    rc = pass(h, kStream | kBin | fe | fixed_flag(h) | (at ? (kATDraw | kATStored) : 0u), pl);   // AT: vel.xyz carries dv between the launches of this call
     if (!rc && emb) rc = emb_md(h);
     if (!rc && emb) rc = emb_bin(h, set, pl.shift);
     if (rc) return rc;
@@ -797,7 +812,7 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
     double *d_ax = d_u + 3 * Nc;
     double *d_kT = d_ax + 3 * Nc;
     int32_t *d_cnt = reinterpret_cast<int32_t *>(d_kT + Nc);
-    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->axis[h->bin_step & 1], h->Nc, h->m, d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
+    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->axis[h->bin_step & 1], h->Nc, h->m, deterministic(h), d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
     h->launches += 1;
     int rc = MPCD_OK;
     auto cp = [&](void *dst, const void *src, size_t b) {
@@ -813,7 +828,8 @@ int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *v
                       int32_t md_substeps)
 {
     if (!h) return MPCD_EINVAL;
-    if (h->opt.rule != MPCD_SRD || thermostatted(h)) return fail(h, MPCD_EINVAL, "embedded beads need the SRD rule without the cell thermostat%s");
+    if (h->opt.rule != MPCD_SRD || thermostatted(h) || deterministic(h))
+        return fail(h, MPCD_EINVAL, "embedded beads need the SRD rule without the cell thermostat and without deterministic accumulation%s");
     if (nb < 1 || !pos3 || !vel3 || !mass || chain_len < 1 || chain_len > kMaxChainLen || nb % chain_len != 0 || !(k >= 0) || !(r0 >= 0) || md_substeps < 1)
         return fail(h, MPCD_EINVAL, "set_embedded: nb >= 1 a multiple of chain_len in [1, 512], k, r0 >= 0, md_substeps >= 1%s");
     std::vector<double4> hp, hv;
@@ -887,7 +903,7 @@ int mpcd_get_thermo(mpcd_t *h, double P[3], double *KE, double *kT)
         if (rc) return rc;
     }
     CUDA_TRY(h, cudaMemsetAsync(h->d_scalars, 0, 8 * sizeof(double), h->stream));
-    cell_thermo<<<h->num_sms * 4, 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->Nc, h->m, h->d_scalars);
+    cell_thermo<<<h->num_sms * 4, 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->Nc, h->m, h->d_scalars, deterministic(h));
     LAUNCH_CHECK(h);
     double out[6];
     CUDA_TRY(h, cudaMemcpyAsync(out, h->d_scalars, sizeof(out), cudaMemcpyDeviceToHost, h->stream));
@@ -906,7 +922,7 @@ int mpcd_get_stats(mpcd_t *h, mpcd_stats *out)
     for (int d = 0; d < 3; ++d) out->n[d] = h->n[d];
     if (h->bin_valid && h->counts_valid) {            // the counts of the last bin are still in its accumulator set
         CUDA_TRY(h, cudaMemsetAsync(h->d_max_occ, 0, sizeof(int), h->stream));
-        cell_max_occupancy<<<h->num_sms * 8, 256, 0, h->stream>>>(h->acc[h->ccur], h->Nc, h->d_max_occ);
+        cell_max_occupancy<<<h->num_sms * 8, 256, 0, h->stream>>>(h->acc[h->ccur], h->Nc, h->d_max_occ, deterministic(h));
         LAUNCH_CHECK(h);
         CUDA_TRY(h, cudaMemcpyAsync(&h->max_occ, h->d_max_occ, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
         CUDA_TRY(h, cudaStreamSynchronize(h->stream));
@@ -958,7 +974,7 @@ int mpcd_abi_version(void) { return MPCD_ABI_VERSION; }
 
 const char *mpcd_build_info(void)
 {
-    return "mpcd-b200 ABI 1, sm_100a, nvcc " __VERSION__
+    return "mpcd-b200 ABI 2, sm_100a, nvcc " __VERSION__
 #ifdef __CUDACC_VER_MAJOR__
            " / CUDA"
 #endif

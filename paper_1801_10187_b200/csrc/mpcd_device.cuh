@@ -5,6 +5,7 @@
 // domain constants are restated here.
 #pragma once
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
 
 namespace mpcdk {
@@ -248,14 +249,48 @@ struct alignas(16) WarpScratch {   // per-warp shared memory of the accumulate p
 #endif
 constexpr int kTreeRounds = MPCD_TREE_ROUNDS;   // rounds of the in-warp combining tree before the REDs; 0 = until one lane per cell is left
 
-template <typename T, bool kCount, bool kEnergy>
+// Deterministic accumulation (the alternative PAPER.md:124-126 mentions): the cell sums are kept
+// as 64-bit fixed-point integers with 40 fractional bits instead of doubles.  Integer addition is associative, so the
+// sums -- and with them the whole trajectory -- no longer depend on the order in which warps and atomics happen to
+// run.  An fp32 velocity is represented exactly whenever |v| >= 2^-17 (absolute rounding error <= 2^-41 otherwise, as
+// for the fp64 value of |v|^2); the range is |sum| < 2^23.  The accumulator words hold the integers' bits.
+constexpr double kFixScale = 1099511627776.0;            // 2^40
+constexpr double kFixInv = 9.094947017729282379150390625e-13;   // 2^-40
+__device__ __forceinline__ long long to_fixed(double x) { return __double2ll_rn(x * kFixScale); }
+__device__ __forceinline__ double fixed_bits(long long x) { return __longlong_as_double(x); }
+// value of an accumulator word: a double, or (fixed) the bits of a fixed-point integer / (count) of a plain integer
+__device__ __forceinline__ double acc_value(double w, bool fixed) { return fixed ? (double)__double_as_longlong(w) * kFixInv : w; }
+__device__ __forceinline__ double acc_count(double w, bool fixed) { return fixed ? (double)__double_as_longlong(w) : w; }
+
+// The combining tree and the transposed REDs, on values of type A: double, or long long for the fixed-point sums.
+template <typename A> struct AccOps;
+template <> struct AccOps<double> {
+    static __device__ __forceinline__ double from(double x) { return x; }
+    static __device__ __forceinline__ double count(int n) { return (double)n; }
+    static __device__ __forceinline__ double stage(double x) { return x; }
+    static __device__ __forceinline__ void red(double *p, double staged) { atomicAdd(p, staged); }
+};
+template <> struct AccOps<long long> {
+    static __device__ __forceinline__ long long from(double x) { return to_fixed(x); }
+    static __device__ __forceinline__ long long count(int n) { return (long long)n; }
+    static __device__ __forceinline__ double stage(long long x) { return fixed_bits(x); }
+    static __device__ __forceinline__ void red(double *p, double staged)
+    {
+        atomicAdd(reinterpret_cast<unsigned long long *>(p), (unsigned long long)__double_as_longlong(staged));
+    }
+};
+
+template <typename T, bool kCount, bool kEnergy, bool kFixed = false>
 __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, double *__restrict__ qacc, WarpScratch &ws,
                                                      int c /* < 0 = inactive lane, unique per lane */, T fx, T fy, T fz)
 {
+    using A = typename std::conditional<kFixed, long long, double>::type;
+    using Ops = AccOps<A>;
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    double vx = (double)fx, vy = (double)fy, vz = (double)fz;
-    double q = kEnergy ? (vx * vx + vy * vy + vz * vz) : 0.0;
+    const double dx0 = (double)fx, dy0 = (double)fy, dz0 = (double)fz;
+    A vx = Ops::from(dx0), vy = Ops::from(dy0), vz = Ops::from(dz0);
+    A q = kEnergy ? Ops::from(dx0 * dx0 + dy0 * dy0 + dz0 * dz0) : A(0);
     unsigned peers = __match_any_sync(full, c);
     const int size = __popc(peers);
     const int rank0 = __popc(peers & ((1u << lane) - 1u));
@@ -269,8 +304,8 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
         alive = !(rank & 1);
         if (next && alive) {
             const double dx = (double)tx, dy = (double)ty, dz = (double)tz;
-            vx += dx; vy += dy; vz += dz;
-            if (kEnergy) q += dx * dx + dy * dy + dz * dz;
+            vx += Ops::from(dx); vy += Ops::from(dy); vz += Ops::from(dz);
+            if (kEnergy) q += Ops::from(dx * dx + dy * dy + dz * dz);
         }
         rounds = 1;
         if (kTreeRounds != 1) {
@@ -282,8 +317,8 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
         while ((kTreeRounds == 0 || rounds < kTreeRounds) && __any_sync(full, alive && peers != 0u)) {   // log2(largest group) rounds at most
             const int next = __ffs(peers);
             const int src = next ? next - 1 : lane;
-            const double tx = __shfl_sync(full, vx, src), ty = __shfl_sync(full, vy, src), tz = __shfl_sync(full, vz, src);
-            const double tq = kEnergy ? __shfl_sync(full, q, src) : 0.0;
+            const A tx = __shfl_sync(full, vx, src), ty = __shfl_sync(full, vy, src), tz = __shfl_sync(full, vz, src);
+            const A tq = kEnergy ? __shfl_sync(full, q, src) : A(0);
             if (next && alive && !(rank & 1)) { vx += tx; vy += ty; vz += tz; q += tq; }
             alive = alive && !(rank & 1);
             peers &= __ballot_sync(full, alive);
@@ -298,18 +333,18 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
     const int nl = __popc(leaders);
     if (alive && c >= 0) {
         const int j = __popc(leaders & ((1u << lane) - 1u));
-        ws.v[0][j] = vx; ws.v[1][j] = vy; ws.v[2][j] = vz;
-        if (kCount) ws.v[3][j] = (double)mine;
-        if (kEnergy) ws.q[j] = q;
+        ws.v[0][j] = Ops::stage(vx); ws.v[1][j] = Ops::stage(vy); ws.v[2][j] = Ops::stage(vz);
+        if (kCount) ws.v[3][j] = Ops::stage(Ops::count(mine));
+        if (kEnergy) ws.q[j] = Ops::stage(q);
         ws.cell[j] = c;
     }
     __syncwarp();
     const int comp = lane & 3;                             // 8 leaders per round, 4 lanes x 8 B = one 32-byte sector each
     for (int base = 0; base < nl; base += 8) {
         const int j = base + (lane >> 2);
-        if (j < nl && (kCount || comp < 3)) atomicAdd(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[comp][j]);
+        if (j < nl && (kCount || comp < 3)) Ops::red(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[comp][j]);
     }
-    if (kEnergy && lane < nl) atomicAdd(qacc + ws.cell[lane], ws.q[lane]);
+    if (kEnergy && lane < nl) Ops::red(qacc + ws.cell[lane], ws.q[lane]);
     __syncwarp();
 }
 

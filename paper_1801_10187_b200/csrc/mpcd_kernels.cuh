@@ -17,6 +17,8 @@
 //                    next kATApply takes it from there instead of regenerating it: one Gaussian draw per particle-step
 //   kEmbedded a5     with kSRD: the cell mean is mass-weighted over the solvent sums and the embedded beads' sums
 //                    (mpcd_embedded.cuh)
+//   kFixed    a4     deterministic accumulation: the cell sums are 64-bit fixed-point integers (mpcd_device.cuh), both
+//                    where they are accumulated (kBin) and where they are read (kSRD)
 //   kSortOut  a8     sort by cell on the way out: instead of in place, the particle is written
 //                    to slot cell_start[c] + (atomic cursor) of the duplicate arrays, c = its cell in the step
 //                    being collided; the separate read-and-scatter pass of the sort disappears
@@ -32,7 +34,7 @@
 
 namespace mpcdk {
 
-enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u, kEmbedded = 512u };
+enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u, kEmbedded = 512u, kFixed = 1024u };
 
 template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
@@ -119,8 +121,9 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     if ((F & kSortOut) && valid) o = atomicAdd(a.cursor + c, 1); // issued early: its latency hides behind the gather
     if (F & kSRD) {
         if (valid) {
-            const f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);    // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
+            f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);          // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
             const f64x4 n = ld256_nc(a.axis + 4 * (size_t)c);
+            if (F & kFixed) { s.x = acc_value(s.x, true); s.y = acc_value(s.y, true); s.z = acc_value(s.z, true); s.w = acc_count(s.w, true); }
             double ux, uy, uz;
             if (F & kEmbedded) {
                 embedded_mean(s, ld256_nc(a.esum + 4 * (size_t)c), a.mass, ux, uy, uz);
@@ -183,7 +186,7 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     }
     if ((F & (kSRD | kATApply | kBin)) && valid) store4(((F & kSortOut) ? a.vel_out : a.vel) + o, vs);
     if ((F & kSortOut) && valid) a.tag_out[o] = tag;
-    if (F & kBin) warp_cell_accumulate<T, true, (F & kEnergy) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
+    if (F & kBin) warp_cell_accumulate<T, true, (F & kEnergy) != 0, (F & kFixed) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
     if (F & kATDraw) warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, ex, ey, ez);
 }
 
@@ -223,15 +226,16 @@ __global__ void __launch_bounds__(256) cell_prepare(double *axis, uint64_t seed,
 // from the canonical distribution; xi = 1 for N_c < 2 and for E_k = 0.  Written into the 4th word of the cell's
 // axis sector, which the collision gathers anyway.
 __global__ void __launch_bounds__(256) cell_thermostat(const double *acc, const double *qacc, double *axis, int64_t Nc, double m, double kT,
-                                                       uint64_t seed, uint64_t step)
+                                                       uint64_t seed, uint64_t step, bool fixed)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
-    const f64x4 s = ld256(acc + 4 * c);
+    f64x4 s = ld256(acc + 4 * c);
+    s.x = acc_value(s.x, fixed); s.y = acc_value(s.y, fixed); s.z = acc_value(s.z, fixed); s.w = acc_count(s.w, fixed);
     const int n = (int)s.w;
     double xi = 1.0;
     if (n >= 2) {
-        const double erel = 0.5 * m * (qacc[c] - (s.x * s.x + s.y * s.y + s.z * s.z) / s.w);
+        const double erel = 0.5 * m * (acc_value(qacc[c], fixed) - (s.x * s.x + s.y * s.y + s.z * s.z) / s.w);
         const double ehat = draw_cell_energy(seed, step, (uint32_t)c, n, kT);
         if (erel > 0.0) xi = sqrt(ehat / erel);
     }
@@ -239,11 +243,11 @@ __global__ void __launch_bounds__(256) cell_thermostat(const double *acc, const 
 }
 
 // Largest cell occupancy of a bin (mpcd_get_stats), from the counts in the accumulator set.
-__global__ void __launch_bounds__(256) cell_max_occupancy(const double *acc, int64_t Nc, int *out)
+__global__ void __launch_bounds__(256) cell_max_occupancy(const double *acc, int64_t Nc, int *out, bool fixed)
 {
     int nmax = 0;
     for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c < Nc; c += (int64_t)gridDim.x * blockDim.x) {
-        const int n = (int)acc[4 * c + 3];
+        const int n = (int)acc_count(acc[4 * c + 3], fixed);
         nmax = n > nmax ? n : nmax;
     }
     nmax = __reduce_max_sync(0xffffffffu, nmax);
@@ -252,13 +256,14 @@ __global__ void __launch_bounds__(256) cell_max_occupancy(const double *acc, int
 
 // a9. Net momentum, kinetic energy, pooled temperature by device-wide reduction.
 // out = {sum Sx, sum Sy, sum Sz, sum Q, sum E_rel over N_c >= 2, sum 1.5 (N_c - 1)}
-__global__ void __launch_bounds__(256) cell_thermo(const double *acc, const double *qacc, int64_t Nc, double m, double *out)
+__global__ void __launch_bounds__(256) cell_thermo(const double *acc, const double *qacc, int64_t Nc, double m, double *out, bool fixed)
 {
     double v[6] = {0, 0, 0, 0, 0, 0};
     for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c < Nc; c += (int64_t)gridDim.x * blockDim.x) {
-        const double2 s0 = reinterpret_cast<const double2 *>(acc + 4 * c)[0];
-        const double2 s1 = reinterpret_cast<const double2 *>(acc + 4 * c)[1];
-        const double q = qacc[c], dn = s1.y;
+        double2 s0 = reinterpret_cast<const double2 *>(acc + 4 * c)[0];
+        double2 s1 = reinterpret_cast<const double2 *>(acc + 4 * c)[1];
+        s0.x = acc_value(s0.x, fixed); s0.y = acc_value(s0.y, fixed); s1.x = acc_value(s1.x, fixed); s1.y = acc_count(s1.y, fixed);
+        const double q = acc_value(qacc[c], fixed), dn = s1.y;
         v[0] += s0.x; v[1] += s0.y; v[2] += s1.x; v[3] += q;
         if (dn >= 2.0) {
             v[4] += 0.5 * m * (q - (s0.x * s0.x + s0.y * s0.y + s1.x * s1.x) / dn);
@@ -271,23 +276,25 @@ __global__ void __launch_bounds__(256) cell_thermo(const double *acc, const doub
 // Unpack the cell arrays for mpcd_get_cells (SoA outputs on the device, copied by the host): u = S / N_c
 // (PAPER.md:122), the cell temperature kT_c = 2 E_rel / (3 (N_c - 1)), E_rel = KE - M_c u^2 / 2
 // (eq. 3; A11, A12).
-__global__ void __launch_bounds__(256) cell_unpack(const double *acc, const double *qacc, const double *axis, int64_t Nc, double m,
+__global__ void __launch_bounds__(256) cell_unpack(const double *acc, const double *qacc, const double *axis, int64_t Nc, double m, bool fixed,
                                                    int32_t *count, double *sumv3, double *ke, double *u3, double *axis3, double *kTc)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
-    const double dn = acc[4 * c + 3];
+    const double dn = acc_count(acc[4 * c + 3], fixed);
+    const double S[3] = {acc_value(acc[4 * c], fixed), acc_value(acc[4 * c + 1], fixed), acc_value(acc[4 * c + 2], fixed)};
+    const double qc = acc_value(qacc[c], fixed);
     double u[3] = {0, 0, 0};
-    if (dn > 0.0) { u[0] = acc[4 * c] / dn; u[1] = acc[4 * c + 1] / dn; u[2] = acc[4 * c + 2] / dn; }
+    if (dn > 0.0) { u[0] = S[0] / dn; u[1] = S[1] / dn; u[2] = S[2] / dn; }
     if (count) count[c] = (int32_t)dn;
-    if (sumv3) { sumv3[3 * c] = acc[4 * c]; sumv3[3 * c + 1] = acc[4 * c + 1]; sumv3[3 * c + 2] = acc[4 * c + 2]; }
-    if (ke) ke[c] = 0.5 * m * qacc[c];
+    if (sumv3) { sumv3[3 * c] = S[0]; sumv3[3 * c + 1] = S[1]; sumv3[3 * c + 2] = S[2]; }
+    if (ke) ke[c] = 0.5 * m * qc;
     if (u3) { u3[3 * c] = u[0]; u3[3 * c + 1] = u[1]; u3[3 * c + 2] = u[2]; }
     if (axis3) { axis3[3 * c] = axis[4 * c]; axis3[3 * c + 1] = axis[4 * c + 1]; axis3[3 * c + 2] = axis[4 * c + 2]; }
     if (kTc) {
         double kT = 0.0;
         if (dn >= 2.0) {
-            const double erel = 0.5 * m * (qacc[c] - dn * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
+            const double erel = 0.5 * m * (qc - dn * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]));
             kT = 2.0 * erel / (3.0 * (dn - 1.0));
         }
         kTc[c] = kT;
@@ -301,14 +308,14 @@ __global__ void __launch_bounds__(256) cell_unpack(const double *acc, const doub
 // ---------------------------------------------------------------------------------------
 constexpr int kScanThreads = 256, kScanItems = 16, kScanTile = kScanThreads * kScanItems;
 
-__global__ void __launch_bounds__(kScanThreads) scan_tile_sums(const double *acc, int64_t Nc, int32_t *tile_sum)
+__global__ void __launch_bounds__(kScanThreads) scan_tile_sums(const double *acc, int64_t Nc, int32_t *tile_sum, bool fixed)
 {
     __shared__ int sm[kScanThreads / 32];
     const int64_t base = (int64_t)blockIdx.x * kScanTile;
     int s = 0;
     for (int k = 0; k < kScanItems; ++k) {
         const int64_t c = base + (int64_t)k * kScanThreads + threadIdx.x;
-        if (c < Nc) s += (int)acc[4 * c + 3];
+        if (c < Nc) s += (int)acc_count(acc[4 * c + 3], fixed);
     }
     s = __reduce_add_sync(0xffffffffu, s);
     if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
@@ -346,7 +353,7 @@ __global__ void __launch_bounds__(1024) scan_tile_offsets(int32_t *tile_sum, int
     }
 }
 
-__global__ void __launch_bounds__(kScanThreads) scan_cells(const double *acc, int64_t Nc, const int32_t *tile_off, int32_t *cell_start)
+__global__ void __launch_bounds__(kScanThreads) scan_cells(const double *acc, int64_t Nc, const int32_t *tile_off, int32_t *cell_start, bool fixed)
 {
     // thread t owns kScanItems consecutive cells of the tile
     __shared__ int sm[kScanThreads];
@@ -354,7 +361,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_cells(const double *acc, in
     int x[kScanItems];
     int s = 0;
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) { x[k] = (base + k < Nc) ? (int)acc[4 * (base + k) + 3] : 0; s += x[k]; }
+    for (int k = 0; k < kScanItems; ++k) { x[k] = (base + k < Nc) ? (int)acc_count(acc[4 * (base + k) + 3], fixed) : 0; s += x[k]; }
     sm[threadIdx.x] = s;
     __syncthreads();
     for (int o = 1; o < kScanThreads; o <<= 1) {

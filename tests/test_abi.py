@@ -41,7 +41,7 @@ def test_north_star_entry_points_present(lib):
 
 def test_abi_version_and_defaults(lib):
     from paper_1801_10187_b200.binding import Options
-    assert lib.mpcd_abi_version() == 1
+    assert lib.mpcd_abi_version() == 2
     assert b"sm_100a" in lib.mpcd_build_info()
     o = Options()
     assert lib.mpcd_default_options(C.byref(o)) == 0
