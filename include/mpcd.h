@@ -116,12 +116,15 @@ int mpcd_stream(mpcd_t *h);
 /* a2-a5. For the current step counter t: draw the grid shift from
  * Philox(seed, t) (A4, A5), bin every particle with the shift
  * applied during binning only (A6), accumulate per cell the count,
- * sum of velocities and kinetic energy in fp64, then per cell
- * the mean velocity u, the relative kinetic energy / temperature (eq. 3
- * PAPER.md:47; A11) and the random unit axis from Philox(seed, t, cell) by
- * cylindrical projection (A13).  Idempotent for a given
- * (state, t).  Direct fp64 accumulation has no capacity, so the overflow /
- * rebuild path of PAPER.md:110 does not exist. */
+ * sum of velocities and kinetic energy in fp64, and draw per cell
+ * the random unit axis from Philox(seed, t, cell) by cylindrical projection
+ * (A13).  The mean velocity u = S / N_c and the cell temperature
+ * (eq. 3; A11) are functions of those sums: the collision forms u where
+ * it uses it, mpcd_get_cells / mpcd_get_thermo report both.  With the thermostat
+ * on, also the scale factor xi of every cell; with embedded beads,
+ * their binning and mass-weighted sums.  Idempotent for a given (state, t).  Direct
+ * accumulation has no capacity, so the overflow / rebuild path of PAPER.md:110 does
+ * not exist. */
 int mpcd_shift_and_bin(mpcd_t *h);
 
 /* a6. SRD collision, eq. 2 / Algorithm 1, angle alpha in
@@ -143,8 +146,9 @@ int mpcd_sort(mpcd_t *h);
 /* nsteps x { stream; shift_and_bin; sort if sort_period and t % sort_period == 0;
  * collide per opt.rule; t += 1 } (A3).  Internally the collision of
  * step t is fused with the streaming / binning / accumulation of step t + 1
- * (one pass over the particles per step); the result is the same as the unfused
- * sequence of calls up to fp64 summation order. */
+ * (one pass over the particles per step), and on sort steps that pass also writes
+ * the particles out in cell order; the result is the same as the unfused sequence
+ * of calls up to fp64 summation order (exactly the same with opt.deterministic). */
 int mpcd_step(mpcd_t *h, int32_t nsteps);
 
 /* Copies the particle state to caller-owned HOST buffers (any may be NULL):
