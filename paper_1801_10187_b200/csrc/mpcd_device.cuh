@@ -233,6 +233,9 @@ struct alignas(16) WarpScratch {   // per-warp shared memory of the accumulate p
     double q[32];
     int cell[32];                  // cell index of leader slot j
 };
+struct alignas(16) WarpScratchX : WarpScratch {   // ... with room for a second triple summed over the same groups (kExtra)
+    double x[3][kStagePitch];
+};
 
 // ---------------------------------------------------------------------------------------
 // Per-cell fp64 accumulation.  Layout in HBM: acc[c] = {Sx, Sy, Sz, N}
@@ -280,10 +283,15 @@ template <> struct AccOps<long long> {
     }
 };
 
-template <typename T, bool kCount, bool kEnergy, bool kFixed = false>
-__device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, double *__restrict__ qacc, WarpScratch &ws,
-                                                     int c /* < 0 = inactive lane, unique per lane */, T fx, T fy, T fz)
+// kExtra: a second triple (ex, ey, ez), already double, is summed over the same groups into xacc[c] = {X, Y, Z, -} by the
+// same match and the same tree (the AT rule's sum of the thermostat draws), instead of a second pass.
+template <typename T, bool kCount, bool kEnergy, bool kFixed = false, bool kExtra = false>
+__device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, double *__restrict__ qacc,
+                                                     typename std::conditional<kExtra, WarpScratchX, WarpScratch>::type &ws,
+                                                     int c /* < 0 = inactive lane, unique per lane */, T fx, T fy, T fz,
+                                                     double *__restrict__ xacc = nullptr, double ex = 0.0, double ey = 0.0, double ez = 0.0)
 {
+    static_assert(!(kExtra && kFixed), "the second triple is summed in double");
     using A = typename std::conditional<kFixed, long long, double>::type;
     using Ops = AccOps<A>;
     const unsigned full = 0xffffffffu;
@@ -302,10 +310,13 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
         const int src = next ? next - 1 : lane;
         const T tx = __shfl_sync(full, fx, src), ty = __shfl_sync(full, fy, src), tz = __shfl_sync(full, fz, src);
         alive = !(rank & 1);
+        const double ux = kExtra ? __shfl_sync(full, ex, src) : 0.0, uy = kExtra ? __shfl_sync(full, ey, src) : 0.0,
+                     uz = kExtra ? __shfl_sync(full, ez, src) : 0.0;
         if (next && alive) {
             const double dx = (double)tx, dy = (double)ty, dz = (double)tz;
             vx += Ops::from(dx); vy += Ops::from(dy); vz += Ops::from(dz);
             if (kEnergy) q += Ops::from(dx * dx + dy * dy + dz * dz);
+            if (kExtra) { ex += ux; ey += uy; ez += uz; }
         }
         rounds = 1;
         if (kTreeRounds != 1) {
@@ -319,7 +330,9 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
             const int src = next ? next - 1 : lane;
             const A tx = __shfl_sync(full, vx, src), ty = __shfl_sync(full, vy, src), tz = __shfl_sync(full, vz, src);
             const A tq = kEnergy ? __shfl_sync(full, q, src) : A(0);
-            if (next && alive && !(rank & 1)) { vx += tx; vy += ty; vz += tz; q += tq; }
+            const double ux = kExtra ? __shfl_sync(full, ex, src) : 0.0, uy = kExtra ? __shfl_sync(full, ey, src) : 0.0,
+                         uz = kExtra ? __shfl_sync(full, ez, src) : 0.0;
+            if (next && alive && !(rank & 1)) { vx += tx; vy += ty; vz += tz; q += tq; if (kExtra) { ex += ux; ey += uy; ez += uz; } }
             alive = alive && !(rank & 1);
             peers &= __ballot_sync(full, alive);
             rank >>= 1;
@@ -336,6 +349,7 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
         ws.v[0][j] = Ops::stage(vx); ws.v[1][j] = Ops::stage(vy); ws.v[2][j] = Ops::stage(vz);
         if (kCount) ws.v[3][j] = Ops::stage(Ops::count(mine));
         if (kEnergy) ws.q[j] = Ops::stage(q);
+        if constexpr (kExtra) { ws.x[0][j] = ex; ws.x[1][j] = ey; ws.x[2][j] = ez; }
         ws.cell[j] = c;
     }
     __syncwarp();
@@ -343,6 +357,7 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
     for (int base = 0; base < nl; base += 8) {
         const int j = base + (lane >> 2);
         if (j < nl && (kCount || comp < 3)) Ops::red(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[comp][j]);
+        if constexpr (kExtra) { if (j < nl && comp < 3) atomicAdd(xacc + 4 * (size_t)ws.cell[j] + comp, ws.x[comp][j]); }
     }
     if (kEnergy && lane < nl) Ops::red(qacc + ws.cell[lane], ws.q[lane]);
     __syncwarp();

@@ -95,8 +95,9 @@ template <typename T, unsigned F>
 __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(const PassArgs<T> a)
 {
     using V4 = typename Vec4<T>::type;
-    __shared__ WarpScratch ws[(F & (kBin | kATDraw)) ? kPassThreads / 32 : 1];
-    WarpScratch &w = ws[(F & (kBin | kATDraw)) ? (threadIdx.x >> 5) : 0];
+    using WS = typename std::conditional<(F & kBin) && (F & kATDraw), WarpScratchX, WarpScratch>::type;
+    __shared__ WS ws[(F & (kBin | kATDraw)) ? kPassThreads / 32 : 1];
+    WS &w = ws[(F & (kBin | kATDraw)) ? (threadIdx.x >> 5) : 0];
     const int64_t i = (int64_t)blockIdx.x * kPassThreads + threadIdx.x;
     const bool valid = i < a.N;
     const int inactive = -1 - (int)(threadIdx.x & 31);
@@ -186,8 +187,10 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     }
     if ((F & (kSRD | kATApply | kBin)) && valid) store4(((F & kSortOut) ? a.vel_out : a.vel) + o, vs);
     if ((F & kSortOut) && valid) a.tag_out[o] = tag;
-    if (F & kBin) warp_cell_accumulate<T, true, (F & kEnergy) != 0, (F & kFixed) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
-    if (F & kATDraw) warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, ex, ey, ez);
+    if constexpr ((F & kBin) && (F & kATDraw))          // one match and one tree for both sums: same cell, same groups
+        warp_cell_accumulate<T, true, (F & kEnergy) != 0, false, true>(a.acc, a.qacc, w, c, v.x, v.y, v.z, a.at_acc, ex, ey, ez);
+    else if constexpr ((F & kBin) != 0) warp_cell_accumulate<T, true, (F & kEnergy) != 0, (F & kFixed) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
+    else if constexpr ((F & kATDraw) != 0) warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, ex, ey, ez);
 }
 
 // Cell index of every particle (the cache in vel.w) as an int32 array, on demand (mpcd_get_state, mpcd_device_ptrs).
