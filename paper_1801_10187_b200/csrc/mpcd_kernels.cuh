@@ -112,16 +112,17 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
             prefetch_l2(base + 128 * (lane < kLines ? lane : lane - kLines));
         }
     }
-    if (valid) {
-        v = load4(a.vel + i);
-        if (F & (kStream | kBin)) p = load4(a.pos + i);
-        if ((F & (kATDraw | kSortOut)) || ((F & kATApply) && !(F & kATStored))) tag = a.tag[i];
-    }
-    int c = valid ? w_to_cell(v.w) : inactive;                   // cell of the last binning (the step being collided)
+    // Lanes past the end of the array (last block only) work on a copy of the last particle and simply do not store or
+    // accumulate: no branch around the loads, the gather and the arithmetic, so the compiler schedules them as one block.
+    const int64_t il = valid ? i : a.N - 1;
+    v = load4(a.vel + il);
+    if (F & (kStream | kBin)) p = load4(a.pos + il);
+    if ((F & (kATDraw | kSortOut)) || ((F & kATApply) && !(F & kATStored))) tag = a.tag[il];
+    int c = w_to_cell(v.w);                                      // cell of the last binning (the step being collided)
     int64_t o = i;                                               // where this particle is written
     if ((F & kSortOut) && valid) o = atomicAdd(a.cursor + c, 1); // issued early: its latency hides behind the gather
     if (F & kSRD) {
-        if (valid) {
+        {
             f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);          // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
             const f64x4 n = ld256_nc(a.axis + 4 * (size_t)c);
             if (F & kFixed) { s.x = acc_value(s.x, true); s.y = acc_value(s.y, true); s.z = acc_value(s.z, true); s.w = acc_count(s.w, true); }
@@ -143,7 +144,7 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
         }
     }
     if (F & kATApply) {
-        if (valid) {                                             // eq. 4: v = u + dv_i - D / N_c = (S - D) / N_c + dv_i
+        {                                                        // eq. 4: v = u + dv_i - D / N_c = (S - D) / N_c + dv_i
             const f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);
             const f64x4 d = ld256_nc(a.dsum + 4 * (size_t)c);
             const double inv = __drcp_rn(s.w);
@@ -161,21 +162,19 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
         }
     }
     if (F & kStream) {
-        if (valid) {
-            p.x = stream_wrap<T>(p.x, v.x, a.dt, a.L[0]);
-            p.y = stream_wrap<T>(p.y, v.y, a.dt, a.L[1]);
-            p.z = stream_wrap<T>(p.z, v.z, a.dt, a.L[2]);
-            store4(((F & kSortOut) ? a.pos_out : a.pos) + o, p);
-        }
+        p.x = stream_wrap<T>(p.x, v.x, a.dt, a.L[0]);
+        p.y = stream_wrap<T>(p.y, v.y, a.dt, a.L[1]);
+        p.z = stream_wrap<T>(p.z, v.z, a.dt, a.L[2]);
+        if (valid) store4(((F & kSortOut) ? a.pos_out : a.pos) + o, p);
     }
     if (F & kBin) {
-        c = valid ? cell_of<T>(p, a.shift, a.inv_a, a.n) : inactive;
+        c = cell_of<T>(p, a.shift, a.inv_a, a.n);
         v.w = cell_to_w(c, T(0));
     }
     V4 vs = v;                                                   // what goes back to the velocity array
     double ex = 0, ey = 0, ez = 0;                               // dv_i of the step being binned
     if (F & kATDraw) {
-        if (valid) {
+        {
             double g0, g1, g2;
             draw_gauss3<T>(a.seed, a.step_bin, tag, g0, g1, g2);
             ex = a.sigma * g0; ey = a.sigma * g1; ez = a.sigma * g2;
@@ -187,6 +186,7 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     }
     if ((F & (kSRD | kATApply | kBin)) && valid) store4(((F & kSortOut) ? a.vel_out : a.vel) + o, vs);
     if ((F & kSortOut) && valid) a.tag_out[o] = tag;
+    if (!valid) c = inactive;                                    // takes no part in the sums
     if constexpr ((F & kBin) && (F & kATDraw))          // one match and one tree for both sums: same cell, same groups
         warp_cell_accumulate<T, true, (F & kEnergy) != 0, false, true>(a.acc, a.qacc, w, c, v.x, v.y, v.z, a.at_acc, ex, ey, ez);
     else if constexpr ((F & kBin) != 0) warp_cell_accumulate<T, true, (F & kEnergy) != 0, (F & kFixed) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
