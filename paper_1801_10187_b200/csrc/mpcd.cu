@@ -54,7 +54,6 @@ struct mpcd {
     int *d_max_occ = nullptr;
     double *d_scalars = nullptr;   // 8 doubles of scratch for reductions
     int ccur = 0;                  // accumulator set of the current bin
-    int64_t prefetch_blocks = 0;   // L2 prefetch distance of the particle pass, in blocks
     int num_sms = 148;
     bool debug_sync = false;       // MPCD_DEBUG_SYNC=1: synchronise after every launch (see LAUNCH_CHECK)
     bool zeroed[2] = {false, false}, at_zeroed[2] = {false, false};
@@ -202,7 +201,6 @@ template <typename T> PassArgs<T> make_args(mpcd_t *h, const PassPlan &pl)
     a.cursor = h->cell_start;
     a.N = h->N;
     a.Nc = h->Nc;
-    a.prefetch = h->prefetch_blocks * (int64_t)kPassThreads;
     for (int d = 0; d < 3; ++d) {
         a.n[d] = h->n[d];
         a.L[d] = (T)h->box[d];
@@ -571,7 +569,6 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
     h->stream = static_cast<cudaStream_t>(o.stream);
     for (int d = 0; d < 3; ++d) { h->n[d] = n[d]; h->box[d] = box[d]; }
     h->Nc = (int64_t)n[0] * n[1] * n[2];
-    if (const char *e = std::getenv("MPCD_PREFETCH_BLOCKS")) h->prefetch_blocks = std::atoll(e);
     if (const char *e = std::getenv("MPCD_DEBUG_SYNC")) h->debug_sync = std::atoi(e) != 0;
     {
         int dev = 0, sms = 0;

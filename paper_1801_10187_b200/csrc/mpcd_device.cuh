@@ -177,7 +177,6 @@ __device__ __forceinline__ void store4(double4 *p, double4 v)
     reinterpret_cast<double2 *>(p)[1] = double2{v.z, v.w};
 }
 #endif
-__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
 // 32-byte (one full sector) accesses for the per-cell records: sm_100 has 256-bit LDG/STG.
 struct f64x4 { double x, y, z, w; };
@@ -354,7 +353,9 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
     }
     __syncwarp();
     const int comp = lane & 3;                             // 8 leaders per round, 4 lanes x 8 B = one 32-byte sector each
-    for (int base = 0; base < nl; base += 8) {
+#pragma unroll
+    for (int base = 0; base < 32; base += 8) {             // at most 32 leaders; fully unrolled, rounds past nl are predicated off
+        if (base >= nl) break;
         const int j = base + (lane >> 2);
         if (j < nl && (kCount || comp < 3)) Ops::red(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[comp][j]);
         if constexpr (kExtra) { if (j < nl && comp < 3) atomicAdd(xacc + 4 * (size_t)ws.cell[j] + comp, ws.x[comp][j]); }

@@ -56,7 +56,6 @@ template <typename T> struct PassArgs {
     uint32_t *tag_out;
     int32_t *cursor;
     int64_t N, Nc;
-    int64_t prefetch;     // particles ahead of this block whose pos/vel lines are pulled into L2 (0 = off)
     int32_t n[3];
     T dt, L[3], inv_a;
     T shift[3];           // grid shift of the step being binned
@@ -103,15 +102,6 @@ __global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(co
     const int inactive = -1 - (int)(threadIdx.x & 31);
     V4 p = {}, v = {};
     uint32_t tag = 0;
-    if (a.prefetch > 0) {        // the lines a later block will stream: 32 particles x sizeof(V4) per warp and array
-        constexpr int kLines = (int)(32 * sizeof(V4) / 128);
-        const int lane = threadIdx.x & 31;
-        const int64_t j = i - lane + a.prefetch;
-        if (lane < 2 * kLines && j + 32 <= a.N) {
-            const char *base = lane < kLines ? reinterpret_cast<const char *>(a.pos + j) : reinterpret_cast<const char *>(a.vel + j);
-            prefetch_l2(base + 128 * (lane < kLines ? lane : lane - kLines));
-        }
-    }
     // Lanes past the end of the array (last block only) work on a copy of the last particle and simply do not store or
     // accumulate: no branch around the loads, the gather and the arithmetic, so the compiler schedules them as one block.
     const int64_t il = valid ? i : a.N - 1;
