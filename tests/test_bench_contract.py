@@ -1,0 +1,35 @@
+"""bench.py's reference arm (the CPU oracle on the host cores) and its JSON contract, runnable without a GPU."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _run(*args, env=None):
+    e = dict(os.environ)
+    e.update(env or {})
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args], capture_output=True, text=True, timeout=600, env=e)
+    assert p.returncode == 0, p.stderr[-2000:]
+    return p.stdout.strip().splitlines()
+
+
+def test_reference_arm_prints_one_json_line_with_the_contract_keys():
+    lines = _run("--impl", "reference", "--steps", "2", "--warmup", "3", "--ref-particles", "20000")
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == "mpcd_particle_steps_per_s" and d["unit"] == "particle-steps/s"
+    assert d["higher_is_better"] is True and d["scaling"] == "weak" and d["vs_baseline"] is None and d["data"] == "synthetic"
+    assert d["steps"] == 2 and d["warmup"] == 3 and d["n_gpus"] == 1 and d["value"] > 0 and d["ms_per_step"] > 0
+    assert d["config"]["workload"].startswith("C3") and "model" not in d["config"]
+    cb = d["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] == 1 and cb["value"] == d["value"] and "sub-box" in cb["sample"]
+    assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+
+
+def test_reference_arm_other_ranks_exit_quietly_and_configs_are_selectable():
+    assert _run("--impl", "reference", "--steps", "1", "--warmup", "3", "--ref-particles", "5000", env={"RANK": "1", "WORLD_SIZE": "2"}) == []
+    for cfg, word in (("C4", "MPCD-AT"), ("C5", "chains of 50 beads")):
+        d = json.loads(_run("--impl", "reference", "--config", cfg, "--steps", "1", "--warmup", "3", "--ref-particles", "20000")[0])
+        assert d["config"]["workload"].startswith(cfg) and word in d["config"]["workload"]
