@@ -71,15 +71,20 @@ __device__ __forceinline__ void gauss3_from_block(const u32x4 b, double &g0, dou
 // The same three Gaussians evaluated in fp32 for the mixed model (A17 allows it as long as the 1e-5 sigma velocity
 // parity holds; no fast-math intrinsics): absolute error <= ~1e-6 against the fp64 evaluation, by construction:
 //  - radius sqrt(-2 ln U): for U > 1/2 the exact small quantity is w = 1 - U = (2^32 - b - 1/2) 2^-32, so
-//    ln U = log1pf(-w) keeps full RELATIVE accuracy where the radius is small; for U <= 1/2, logf(U) has absolute
-//    error ~6e-8 and the radius is > 1.17;
+//    ln U = log1pf(-w) keeps full RELATIVE accuracy where the radius is small; for U <= 1/2, ln U = log1pf(m - 1) - k ln 2
+//    with the normalised mantissa m has absolute error ~1e-6 at most while the radius is > 1.17;
 //  - angle 2 U1 (in units of pi) = hi + lo with hi the top 24 bits (exact in fp32) and lo < 2^-23 applied as a
 //    first-order rotation of sincospif(hi), instead of rounding U1 itself to 24 bits.
 __device__ __forceinline__ float bm_radius_f32(uint32_t b)
 {
-    float lnu;
-    if (b & 0x80000000u) lnu = log1pf(-((float)(0xffffffffu - b) + 0.5f) * 2.3283064365386962890625e-10f);
-    else lnu = logf(((float)b + 0.5f) * 2.3283064365386962890625e-10f);
+    // One log1pf for both regimes, no divergence: U = m 2^-k with k = clz(b), m in [1/2, 1).  For U > 1/2 (k = 0) the
+    // argument m - 1 = -w is formed from the integer 2^32 - 1 - b and is exact; for U <= 1/2 the mantissa m carries a
+    // relative rounding of 2^-24, harmless there (|ln U| > 0.69).
+    const int k = __clz((int)b);                                            // 0 when the top bit is set; 32 for b = 0
+    const float w = ((float)(0xffffffffu - b) + 0.5f) * 2.3283064365386962890625e-10f;
+    const float m = ((float)(k < 32 ? b << k : 0u) + ldexpf(0.5f, k)) * 2.3283064365386962890625e-10f;
+    const float x = k == 0 ? -w : m - 1.0f;
+    const float lnu = fmaf(-(float)k, 0.693147182464599609375f, log1pf(x));
     return sqrtf(-2.0f * lnu);
 }
 __device__ __forceinline__ void bm_sincos_f32(uint32_t b, float &s, float &c)      // sin, cos of 2 pi (b + 1/2) 2^-32
