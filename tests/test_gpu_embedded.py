@@ -58,6 +58,22 @@ def test_fused_steps_with_beads_match_the_oracle(oracle, dtype):
     assert np.array_equal(e["cell"], o.emb["cell"])
 
 
+def test_step_by_step_equals_one_call_with_beads(oracle):
+    """mpcd_step(1) x 4 (no fused kernel) and mpcd_step(4) (fused kernels, a sort on the way) give the same beads and solvent."""
+    ga, _, _ = _pair(oracle, (8, 8, 8), 5, 44, np.float64, 8, 16, sort_period=2)
+    gb, _, _ = _pair(oracle, (8, 8, 8), 5, 44, np.float64, 8, 16, sort_period=2)
+    ga.step(4)
+    for _ in range(4):
+        gb.step(1)
+    ea, eb = ga.get_embedded(), gb.get_embedded()
+    np.testing.assert_allclose(ea["pos"], eb["pos"], rtol=0, atol=1e-11)
+    np.testing.assert_allclose(ea["vel"], eb["vel"], rtol=0, atol=1e-11)
+    sa, sb = ga.get_state(), gb.get_state()
+    a, b = np.argsort(sa["tag"]), np.argsort(sb["tag"])
+    np.testing.assert_allclose(sa["vel"][a], sb["vel"][b], rtol=0, atol=1e-11)
+    np.testing.assert_allclose(sa["pos"][a], sb["pos"][b], rtol=0, atol=1e-11)
+
+
 def test_config5_like_run_conserves_momentum_and_equilibrates():
     """BASELINE config 5 at reduced size: 32^3 cells, density 5, 100 chains of 50 beads (mass 5, k = 1000, r0 = 0.5),
     10 MD substeps per collision, mixed precision; the beads start twice too hot."""
