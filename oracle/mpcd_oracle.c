@@ -28,7 +28,12 @@
  * fsum; axis statistics; rotation vs scipy Rotation (handedness), RR^T = I;
  * per-cell momentum / energy conservation; one-step decorrelation closed forms;
  * Maxwell-Boltzmann KS test; viscosity 8.7 by transverse-mode
- * decay; AT conservation / Gaussianity / tag-keying; sort multiset + stability.
+ * decay; AT conservation / Gaussianity / tag-keying; sort multiset + stability;
+ * cell thermostat: drawn energies vs scipy's Gamma distribution, E_k' = E^ per cell,
+ * one-collision thermalisation (test_oracle_thermostat.py); embedded solute: the
+ * velocity-Verlet dimer against its closed form, forces vs numerical gradients, MD
+ * momentum / bounded energy, mass-weighted collision invariants, equipartition
+ * (test_oracle_embedded.py).
  * parity unpinned: none.
  */
 #include <math.h>
