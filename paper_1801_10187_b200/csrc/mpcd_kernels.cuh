@@ -87,11 +87,16 @@ __device__ __forceinline__ double cell_to_w(int c, double) { return __longlong_a
 __device__ __forceinline__ int w_to_cell(float w) { return __float_as_int(w); }
 __device__ __forceinline__ int w_to_cell(double w) { return (int)__double_as_longlong(w); }
 
-#ifndef MPCD_MINBLOCKS
-#define MPCD_MINBLOCKS 10     // x 128 threads = 40 warps per SM at <= 51 registers (measured best: DESIGN.md 5.1)
+// Blocks of 128 threads per SM the register count is held to (measured best): 12 (<= 42 registers, 48
+// warps) in the mixed model, 10 (<= 51 registers, 40 warps) in the fp64 model, whose 64-bit state needs the registers.
+#ifndef MPCD_MINBLOCKS_F32
+#define MPCD_MINBLOCKS_F32 12
+#endif
+#ifndef MPCD_MINBLOCKS_F64
+#define MPCD_MINBLOCKS_F64 10
 #endif
 template <typename T, unsigned F>
-__global__ void __launch_bounds__(kPassThreads, MPCD_MINBLOCKS) particle_pass(const PassArgs<T> a)
+__global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_F32 : MPCD_MINBLOCKS_F64) particle_pass(const PassArgs<T> a)
 {
     using V4 = typename Vec4<T>::type;
     using WS = typename std::conditional<(F & kBin) && (F & kATDraw), WarpScratchX, WarpScratch>::type;
