@@ -50,6 +50,8 @@ struct mpcd {
     double *emb_acc[2] = {nullptr, nullptr};
     bool emb_zeroed[2] = {false, false};
     bool emb_binned = false;       // the beads are binned and summed for the current bin
+    cudaStream_t emb_stream = nullptr;   // inside mpcd_step the bead kernel runs beside the solvent's step kernel (fork / join by events)
+    cudaEvent_t emb_fork = nullptr, emb_join = nullptr;
     int32_t *cell_start = nullptr, *tile_sum = nullptr;
     int *d_max_occ = nullptr;
     double *d_scalars = nullptr;   // 8 doubles of scratch for reductions
@@ -387,6 +389,37 @@ int emb_rotate(mpcd_t *h, int cset, uint64_t step_collide, double alpha)
     return MPCD_OK;
 }
 
+// inside mpcd_step: [collide(step_collide) with set cset] + MD + [bin under `shift` into set bset] as one launch
+template <unsigned G> int emb_step_launch(mpcd_t *h, int cset, int bset, uint64_t step_collide, const double shift[3], double alpha, bool beside = false)
+{
+    // beside: on the beads' own stream, after everything enqueued so far on the handle's stream (fork); the caller joins
+    cudaStream_t st = beside && h->emb_stream ? h->emb_stream : h->stream;
+    if (st != h->stream) {
+        CUDA_TRY(h, cudaEventRecord(h->emb_fork, h->stream));
+        CUDA_TRY(h, cudaStreamWaitEvent(st, h->emb_fork, 0));
+    }
+    MdArgs a{};
+    a.pos = h->emb_pos; a.vel = h->emb_vel; a.chain_len = h->emb_chain_len; a.nsub = h->emb_nsub;
+    a.k = h->emb_k; a.r0 = h->emb_r0; a.dt = h->opt.dt / h->emb_nsub;
+    for (int d = 0; d < 3; ++d) a.L[d] = h->box[d];
+    EmbArgs e = emb_args(h, cset, bset, step_collide, shift, alpha);
+    {
+        ProfScope prof(h, MPCD_PROF_OTHER);      // (with `beside` the pair of events on the handle's stream brackets nothing: the count is kept, the time is not)
+        emb_step<G><<<(unsigned)(h->emb_n / h->emb_chain_len), kEmbThreads, (size_t)h->emb_chain_len * 10 * sizeof(double), st>>>(a, e);
+        LAUNCH_CHECK(h);
+    }
+    if (st != h->stream) CUDA_TRY(h, cudaEventRecord(h->emb_join, st));
+    if (G & kEmbBinAcc) h->emb_zeroed[bset] = false;
+    return MPCD_OK;
+}
+
+// the handle's stream waits for the bead kernel launched beside it
+int emb_join_stream(mpcd_t *h)
+{
+    if (h->emb_stream) CUDA_TRY(h, cudaStreamWaitEvent(h->stream, h->emb_join, 0));
+    return MPCD_OK;
+}
+
 // a8, first half: exclusive scan of the per-cell counts of accumulator set `s` -> cell_start (the write cursors)
 int scan_counts(mpcd_t *h, int s)
 {
@@ -498,6 +531,9 @@ int init_state(mpcd_t *h)
 
 void release(mpcd_t *h)
 {
+    if (h->emb_stream) { cudaStreamSynchronize(h->emb_stream); cudaStreamDestroy(h->emb_stream); h->emb_stream = nullptr; }
+    if (h->emb_fork) { cudaEventDestroy(h->emb_fork); h->emb_fork = nullptr; }
+    if (h->emb_join) { cudaEventDestroy(h->emb_join); h->emb_join = nullptr; }
     for (const Buffer &b : h->buffers) {
         if (h->opt.free_fn) h->opt.free_fn(b.ptr, h->opt.alloc_user);
         else if (!h->opt.alloc_fn) cudaFree(b.ptr);
@@ -709,8 +745,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     pl.step_collide = pl.step_bin = t;
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
     rc = pass(h, kStream | kBin | fe | fixed_flag(h) | (at ? (kATDraw | kATStored) : 0u), pl);   // AT: vel.xyz carries dv between the launches of this call
-    if (!rc && emb) rc = emb_md(h);
-    if (!rc && emb) rc = emb_bin(h, set, pl.shift);
+    if (!rc && emb) rc = emb_step_launch<kEmbMd | kEmbBinAcc>(h, set, set, t, pl.shift, h->opt.alpha);
     if (rc) return rc;
     if (ft) { rc = thermostat(h, t); if (rc) return rc; }
     bool sort_pending = sort_due(h, t);            // sort by the cells of step t: done by the next fused kernel on its way out
@@ -721,18 +756,17 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
         rc = prepare(h, nxt, true, at, !at, t + 1);
         if (rc) return rc;
         if (sort_pending) { rc = scan_counts(h, set); if (rc) return rc; }
-        if (emb) {                                  // beads: collide(t) with the complete sums of step t, then MD over the next interval
-            rc = emb_rotate(h, set, t, h->opt.alpha);
-            if (!rc) rc = emb_md(h);
+        shift_for(h, t + 1, pl.shift);
+        if (emb) {            // beads, one launch: collide(t) with the complete sums of step t, MD over the next interval, bin(t + 1)
+            rc = emb_step_launch<kEmbRotate | kEmbMd | kEmbBinAcc>(h, set, nxt, t, pl.shift, h->opt.alpha, true);   // beside the solvent's kernel
             if (rc) return rc;
         }
-        shift_for(h, t + 1, pl.shift);
-        if (emb) { rc = emb_bin(h, nxt, pl.shift); if (rc) return rc; }
         pl.cset = set; pl.bset = nxt;
         pl.step_collide = t; pl.step_bin = t + 1;
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
         rc = pass(h, (at ? (kATApply | kATDraw | kATStored) : (kSRD | ft | fb)) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
         if (rc) return rc;
+        if (emb) { rc = emb_join_stream(h); if (rc) return rc; }
         if (sort_pending) { h->pcur ^= 1; h->sorts += 1; }
         set = nxt; t += 1;
         if (ft) { rc = thermostat(h, t); if (rc) return rc; }
@@ -844,6 +878,13 @@ int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *v
         if (!rc) rc = dev_alloc_t(h, &h->emb_vel, (size_t)nb);
         for (int s = 0; s < 2 && !rc; ++s) { rc = dev_alloc_t(h, &h->emb_acc[s], (size_t)h->Nc * 4); h->emb_zeroed[s] = false; }
         if (rc) return rc;
+        if (cudaStreamCreateWithFlags(&h->emb_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&h->emb_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&h->emb_join, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();                       // no side stream: the bead kernel simply runs in line
+            if (h->emb_stream) cudaStreamDestroy(h->emb_stream);
+            h->emb_stream = nullptr;
+        }
     }
     CUDA_TRY(h, cudaMemcpyAsync(h->emb_pos, hp.data(), (size_t)nb * sizeof(double4), cudaMemcpyHostToDevice, h->stream));
     CUDA_TRY(h, cudaMemcpyAsync(h->emb_vel, hv.data(), (size_t)nb * sizeof(double4), cudaMemcpyHostToDevice, h->stream));

@@ -147,4 +147,86 @@ __global__ void __launch_bounds__(kEmbThreads) emb_collide(const EmbArgs a)
     st_d4(a.vel + i, v);
 }
 
+// The three bead kernels of one step inside mpcd_step as ONE launch (config 5 is half launch-bound: 5 M solvent
+// particles take 0.12 ms per step): per chain block, collide the beads with the complete sums of step t (kRotate), advance
+// them by MD over the next interval (kMd), then bin them under the shift of step t + 1 and add them to that step's
+// bead sums (kBinAcc).  The same arithmetic, in the same order, as emb_collide, emb_md_verlet and emb_bin_accumulate.
+enum : unsigned { kEmbRotate = 1u, kEmbMd = 2u, kEmbBinAcc = 4u };
+
+template <unsigned G>
+__global__ void __launch_bounds__(kEmbThreads) emb_step(const MdArgs a, const EmbArgs e)
+{
+    extern __shared__ double sm[];
+    const int n = a.chain_len;
+    double *sx = sm, *sv = sm + 3 * n, *sf = sm + 6 * n, *smass = sm + 9 * n;
+    const int64_t base = (int64_t)blockIdx.x * n;
+    const double L[3] = {a.L[0], a.L[1], a.L[2]};
+    for (int j = threadIdx.x; j < n; j += kEmbThreads) {
+        const double4 p = ld_d4(a.pos + base + j);
+        double4 v = ld_d4(a.vel + base + j);
+        if (G & kEmbRotate) {
+            const size_t c = (size_t)__double_as_longlong(v.w);
+            const f64x4 s = ld256(e.sums + 4 * c), b = ld256(e.esum + 4 * c), ax = ld256(e.axis + 4 * c);
+            double ux, uy, uz;
+            embedded_mean(s, b, e.mass_solvent, ux, uy, uz);
+            const double wx = v.x - ux, wy = v.y - uy, wz = v.z - uz;
+            const double ndw = ax.x * wx + ax.y * wy + ax.z * wz, omc = 1.0 - e.cos_a;
+            v.x = ux + (wx * e.cos_a + (ax.y * wz - ax.z * wy) * e.sin_a + ax.x * ndw * omc);
+            v.y = uy + (wy * e.cos_a + (ax.z * wx - ax.x * wz) * e.sin_a + ax.y * ndw * omc);
+            v.z = uz + (wz * e.cos_a + (ax.x * wy - ax.y * wx) * e.sin_a + ax.z * ndw * omc);
+        }
+        sx[3 * j] = p.x; sx[3 * j + 1] = p.y; sx[3 * j + 2] = p.z; smass[j] = p.w;
+        sv[3 * j] = v.x; sv[3 * j + 1] = v.y; sv[3 * j + 2] = v.z;
+    }
+    __syncthreads();
+    if (G & kEmbMd) {
+        auto forces = [&]() {
+            for (int j = threadIdx.x; j < n; j += kEmbThreads) {
+                double d[3], g, fx = 0.0, fy = 0.0, fz = 0.0;
+                if (j > 0) { bond(sx + 3 * (j - 1), sx + 3 * j, L, a.k, a.r0, d, g); fx = g * d[0]; fy = g * d[1]; fz = g * d[2]; }
+                if (j + 1 < n) { bond(sx + 3 * j, sx + 3 * (j + 1), L, a.k, a.r0, d, g); fx -= g * d[0]; fy -= g * d[1]; fz -= g * d[2]; }
+                sf[3 * j] = fx; sf[3 * j + 1] = fy; sf[3 * j + 2] = fz;
+            }
+        };
+        forces();
+        for (int s = 0; s < a.nsub; ++s) {
+            __syncthreads();
+            for (int j = threadIdx.x; j < n; j += kEmbThreads) {
+                const double h = 0.5 * a.dt / smass[j];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    sv[3 * j + c] += h * sf[3 * j + c];
+                    double x = sx[3 * j + c] + sv[3 * j + c] * a.dt;
+                    if (x < 0.0) x += L[c];
+                    if (x >= L[c]) x -= L[c];
+                    sx[3 * j + c] = x;
+                }
+            }
+            __syncthreads();
+            forces();
+            for (int j = threadIdx.x; j < n; j += kEmbThreads) {
+                const double h = 0.5 * a.dt / smass[j];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) sv[3 * j + c] += h * sf[3 * j + c];
+            }
+        }
+    }
+    for (int j = threadIdx.x; j < n; j += kEmbThreads) {
+        double4 v = ld_d4(a.vel + base + j);             // keeps .w (the cached cell index) unless the beads are re-binned
+        v.x = sv[3 * j]; v.y = sv[3 * j + 1]; v.z = sv[3 * j + 2];
+        const double4 p = double4{sx[3 * j], sx[3 * j + 1], sx[3 * j + 2], smass[j]};
+        if (G & kEmbBinAcc) {
+            const int ix = bin_axis<double>(p.x, e.shift[0], e.inv_a, e.n[0]);
+            const int iy = bin_axis<double>(p.y, e.shift[1], e.inv_a, e.n[1]);
+            const int iz = bin_axis<double>(p.z, e.shift[2], e.inv_a, e.n[2]);
+            const int c = ix + e.n[0] * (iy + e.n[1] * iz);
+            v.w = __longlong_as_double((long long)c);
+            double *q = e.eacc + 4 * (size_t)c;
+            atomicAdd(q, p.w * v.x); atomicAdd(q + 1, p.w * v.y); atomicAdd(q + 2, p.w * v.z); atomicAdd(q + 3, p.w);
+        }
+        if (G & kEmbMd) st_d4(a.pos + base + j, p);
+        st_d4(a.vel + base + j, v);
+    }
+}
+
 }  // namespace mpcdk
