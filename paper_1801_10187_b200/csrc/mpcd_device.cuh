@@ -234,7 +234,6 @@ template <typename T> __device__ __forceinline__ int bin_axis(T x, T s, T inv_a,
 constexpr int kStagePitch = 36;    // doubles per staged component row: 4 rows land in disjoint banks for one half-warp
 struct alignas(16) WarpScratch {   // per-warp shared memory of the accumulate phase
     double v[4][kStagePitch];      // [component][leader slot]
-    double q[32];
     int cell[32];                  // cell index of leader slot j
 };
 struct alignas(16) WarpScratchX : WarpScratch {   // ... with room for a second triple summed over the same groups (kExtra)
@@ -352,7 +351,7 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
         const int j = __popc(leaders & ((1u << lane) - 1u));
         ws.v[0][j] = Ops::stage(vx); ws.v[1][j] = Ops::stage(vy); ws.v[2][j] = Ops::stage(vz);
         if (kCount) ws.v[3][j] = Ops::stage(Ops::count(mine));
-        if (kEnergy) ws.q[j] = Ops::stage(q);
+        if (kEnergy) Ops::red(qacc + c, Ops::stage(q));    // one 8-byte RED per leader, straight from its registers
         if constexpr (kExtra) { ws.x[0][j] = ex; ws.x[1][j] = ey; ws.x[2][j] = ez; }
         ws.cell[j] = c;
     }
@@ -365,7 +364,6 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
         if (j < nl && (kCount || comp < 3)) Ops::red(acc + 4 * (size_t)ws.cell[j] + comp, ws.v[comp][j]);
         if constexpr (kExtra) { if (j < nl && comp < 3) atomicAdd(xacc + 4 * (size_t)ws.cell[j] + comp, ws.x[comp][j]); }
     }
-    if (kEnergy && lane < nl) Ops::red(qacc + ws.cell[lane], ws.q[lane]);
     __syncwarp();
 }
 
