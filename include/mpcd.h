@@ -39,7 +39,7 @@
 extern "C" {
 #endif
 
-#define MPCD_ABI_VERSION 2
+#define MPCD_ABI_VERSION 3
 
 /* status codes */
 #define MPCD_OK      0
@@ -83,7 +83,12 @@ typedef struct mpcd_options {
                               fixed-point integers (40 fractional bits), so the trajectory is bit-reproducible whatever the order of
                               warps, atomics and particles in memory; results stay within the mixed-model tolerance of the fp64
                               sums.  Mixed model + SRD rule only (MPCD_EINVAL otherwise; no embedded beads); default 0 */
-    int32_t reserved1;
+    int32_t brick;         /* 1 (default): the sort (sect. 3.8) orders the particles BRICK-major -- cells grouped in bricks of
+                              brick[0] x brick[1] x brick[2] cells (mpcd_stats.brick; compile-time), bricks x-fastest over
+                              ceil(n_d / brick[d]) per axis, cells x-fastest inside a brick -- and mpcd_step runs its steady-state kernel
+                              with one thread block per brick and the cell side of the step in shared memory.  The
+                              order inside the sort is free (A20): results are the same up to fp64 summation order.
+                              0: ascending cell index and the warp-level kernel */
     void *stream;          /* cudaStream_t the library enqueues on; NULL = the legacy default stream */
     mpcd_alloc_fn alloc_fn;
     mpcd_free_fn free_fn;
@@ -138,9 +143,13 @@ int mpcd_collide_srd(mpcd_t *h, double alpha);
  * second per-cell reduction, v <- u + dv - sum(dv)/N_c.  Same preconditions. */
 int mpcd_collide_at(mpcd_t *h);
 
-/* a8. Sort by cell, sect. 3.8: reorder pos, vel, tag and cell
- * into ascending cell order using the current bin (MPCD_ESTATE if none).  Order
- * within a cell is unspecified (A20).  Tags travel with particles. */
+/* a8. Sort by cell, sect. 3.8: reorder pos, vel, tag and cell so
+ * that the particles of a cell are contiguous, using the current bin (MPCD_ESTATE
+ * if none).  Cells follow each other in ascending SORT KEY: the cell index with
+ * opt.brick = 0; with opt.brick = 1, for cell (ix, iy, iz) and brick edges
+ * B = mpcd_stats.brick[0..2], nb_d = ceil(n_d / B_d):
+ *   key = (((iz/Bz) nb_y + iy/By) nb_x + ix/Bx) Bx By Bz + ((iz%Bz) By + iy%By) Bx + ix%Bx.
+ * Order within a cell is unspecified (A20).  Tags travel with particles. */
 int mpcd_sort(mpcd_t *h);
 
 /* nsteps x { stream; shift_and_bin; sort if sort_period and t % sort_period == 0;
@@ -203,6 +212,7 @@ typedef struct mpcd_stats {
     uint64_t kernel_launches; /* kernels launched by this handle so far */
     uint64_t sorts;         /* sorts done so far */
     uint64_t device_bytes;  /* bytes obtained from the allocator */
+    int32_t brick[4];       /* brick edges (cells) per axis and the window halo of the brick kernel; zeros with opt.brick = 0 */
 } mpcd_stats;
 int mpcd_get_stats(mpcd_t *h, mpcd_stats *out /* host */);
 

@@ -28,7 +28,7 @@ class Options(C.Structure):
     _fields_ = [
         ("precision", C.c_int32), ("rule", C.c_int32), ("dt", C.c_double), ("alpha", C.c_double),
         ("sort_period", C.c_int32), ("cell_energy", C.c_int32), ("init_state", C.c_int32), ("thermostat", C.c_int32),
-        ("deterministic", C.c_int32), ("reserved1", C.c_int32),
+        ("deterministic", C.c_int32), ("brick", C.c_int32),
         ("stream", C.c_void_p), ("alloc_fn", ALLOC_FN), ("free_fn", FREE_FN), ("alloc_user", C.c_void_p),
     ]
 
@@ -37,6 +37,7 @@ class Stats(C.Structure):
     _fields_ = [
         ("N", C.c_int64), ("Nc", C.c_int64), ("n", C.c_int32 * 3), ("max_occupancy", C.c_int32),
         ("step", C.c_uint64), ("kernel_launches", C.c_uint64), ("sorts", C.c_uint64), ("device_bytes", C.c_uint64),
+        ("brick", C.c_int32 * 4),
     ]
 
 
@@ -140,7 +141,7 @@ class MPCD:
 
     def __init__(self, box, N, a=1.0, m=1.0, kT=1.0, seed=0, *, precision="mixed", rule="srd", dt=0.1,
                  alpha=math.radians(130.0), sort_period=25, cell_energy=True, init_state=True, thermostat=False, deterministic=False,
-                 device="cuda:0", use_torch_allocator=True, stream=None):
+                 brick=True, device="cuda:0", use_torch_allocator=True, stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1801_10187_b200 needs a CUDA device (no CPU fallback)")
@@ -158,6 +159,7 @@ class MPCD:
         opt.sort_period, opt.cell_energy, opt.init_state = int(sort_period), int(bool(cell_energy)), int(bool(init_state))
         opt.thermostat = int(bool(thermostat))
         opt.deterministic = int(bool(deterministic))
+        opt.brick = int(bool(brick))
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         opt.stream = C.c_void_p(self._stream.cuda_stream)
         self._alloc = TorchAllocator(device) if use_torch_allocator else None
@@ -270,7 +272,7 @@ class MPCD:
         s = Stats()
         self._check(self.lib.mpcd_get_stats(self.h, C.byref(s)))
         return dict(N=s.N, Nc=s.Nc, n=tuple(s.n), max_occupancy=s.max_occupancy, step=s.step,
-                    kernel_launches=s.kernel_launches, sorts=s.sorts, device_bytes=s.device_bytes)
+                    kernel_launches=s.kernel_launches, sorts=s.sorts, device_bytes=s.device_bytes, brick=tuple(s.brick))
 
     def set_profiling(self, on=True):
         self._check(self.lib.mpcd_set_profiling(self.h, int(bool(on))))

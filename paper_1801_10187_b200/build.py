@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmpcd_b200.so")
 SOURCES = ["mpcd.cu"]
-DEPS = ["mpcd.cu", "mpcd_kernels.cuh", "mpcd_device.cuh", os.path.join("..", "..", "include", "mpcd.h")]
+DEPS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh"))) + [os.path.join("..", "..", "include", "mpcd.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

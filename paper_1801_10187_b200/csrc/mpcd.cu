@@ -3,7 +3,7 @@
 // mpcd_kernels.cuh; the only method arithmetic on the host is the three-scalar grid-shift
 // draw (a2) and cos/sin of the SRD angle (A15).
 #include "../../include/mpcd.h"
-#include "mpcd_kernels.cuh"
+#include "mpcd_brick.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -34,6 +34,7 @@ struct mpcd {
     // particle arrays, double-buffered for the sort
     void *pos[2] = {nullptr, nullptr}, *vel[2] = {nullptr, nullptr};
     uint32_t *tag[2] = {nullptr, nullptr};
+    void *cells_stage = nullptr;   // mpcd_get_cells' staging buffer, from the allocator on first use
     int32_t *cell = nullptr;       // cell index per particle, filled on demand only (mpcd_get_state / mpcd_device_ptrs)
     int pcur = 0;
     // cell arrays, double-buffered by step parity: while the fused kernel reads the sums and axes of step t
@@ -53,6 +54,13 @@ struct mpcd {
     cudaStream_t emb_stream = nullptr;   // inside mpcd_step the bead kernel runs beside the solvent's step kernel (fork / join by events)
     cudaEvent_t emb_fork = nullptr, emb_join = nullptr;
     int32_t *cell_start = nullptr, *tile_sum = nullptr;
+    // brick-major sort order and the brick-tiled step kernel (mpcd_brick.cuh)
+    BrickGrid grid{};              // the sort keys: grid.on = 0 is the plain ascending-cell order
+    int32_t nbricks = 0;
+    int32_t *brick_start[2] = {nullptr, nullptr};   // segment starts of the current order / of the sort being prepared
+    int bcur = 0;
+    bool brick_valid = false;      // the particle arrays are in brick-major order of the bin whose shift is brick_shift
+    double brick_shift[3] = {0, 0, 0};
     int *d_max_occ = nullptr;
     double *d_scalars = nullptr;   // 8 doubles of scratch for reductions
     int ccur = 0;                  // accumulator set of the current bin
@@ -173,6 +181,17 @@ void draw_shift(const mpcd_t *h, uint64_t step, double s[3])
     for (int d = 0; d < 3; ++d) s[d] = (u01_32(w[d]) - 0.5) * h->a;
 }
 
+inline bool thermostatted(const mpcd_t *h) { return h->opt.thermostat != 0; }
+inline bool deterministic(const mpcd_t *h) { return h->opt.deterministic != 0; }
+inline unsigned fixed_flag(const mpcd_t *h) { return h->opt.deterministic != 0 ? kFixed : 0u; }
+
+// the shift as the binning applies it
+inline void shift_for(const mpcd_t *h, uint64_t step, double out[3])
+{
+    draw_shift(h, step, out);
+    if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) out[d] = (double)(float)out[d];   // A5
+}
+
 // What one launch of the pass works on: `cset` = accumulator set of the step being collided (its sums, thermostat
 // sums and, by step parity, its axes), `bset` = set of the step being binned.
 struct PassPlan {
@@ -279,10 +298,71 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
     return MPCD_OK;
 }
 
+// The brick kernel's view of one launch: the segment starts of the current order, where the two cell windows sit
+// relative to a brick (the shift of the step collided / binned against the shift of the bin the arrays were sorted by,
+// centred on the halo), and the fixed-point scales of the shared-memory partial sums (mpcd_brick.cuh).
+BrickArgs brick_args(const mpcd_t *h, const PassPlan &pl)
+{
+    BrickArgs g{};
+    g.brick_start = h->brick_start[h->bcur];
+    double sc[3];
+    shift_for(h, pl.step_collide, sc);
+    for (int d = 0; d < 3; ++d) {
+        g.nb[d] = h->grid.nb[d];
+        g.og[d] = (int32_t)std::floor((sc[d] - h->brick_shift[d]) / h->a - 0.5 * kH + 0.5);
+        g.oa[d] = (int32_t)std::floor((pl.shift[d] - h->brick_shift[d]) / h->a - 0.5 * kH + 0.5);
+    }
+    g.div_nx = make_div31((uint32_t)h->n[0]);
+    g.div_nxy = make_div31((uint32_t)h->n[0] * (uint32_t)h->n[1]);
+    int e = 0;
+    std::frexp(h->sigma, &e);                        // unit = 2^e >= sqrt(kT / m)
+    if (deterministic(h)) {
+        g.sv = g.sq = kFixScale; g.inv_sv = g.inv_sq = kFixInv; g.vmax = HUGE_VAL;
+    } else {
+        g.sv = std::ldexp(1.0, 48 - e); g.inv_sv = std::ldexp(1.0, e - 48);
+        g.sq = std::ldexp(1.0, 44 - 2 * e); g.inv_sq = std::ldexp(1.0, 2 * e - 44);
+        g.vmax = std::ldexp(8.0, e);
+    }
+    return g;
+}
+
+template <typename T> int launch_brick(mpcd_t *h, unsigned F, const PassPlan &pl)
+{
+    const PassArgs<T> a = make_args<T>(h, pl);
+    const BrickArgs g = brick_args(h, pl);
+    switch (F) {
+#define CASE(f) case (f): brick_pass<T, (f)><<<(unsigned)h->nbricks, kBrickThreads, 0, h->stream>>>(a, g); break;
+#define CASE_F32(f) case (f): if constexpr (sizeof(T) == 4) { brick_pass<T, (f)><<<(unsigned)h->nbricks, kBrickThreads, 0, h->stream>>>(a, g); break; } else return fail(h, MPCD_EINVAL, "internal: fixed-point sums need the mixed model%s");
+        CASE(kSRD | kStream | kBin)
+        CASE(kSRD | kStream | kBin | kEnergy)
+        CASE(kSRD | kStream | kBin | kSortOut)
+        CASE(kSRD | kStream | kBin | kEnergy | kSortOut)
+        CASE(kSRD | kEmbedded | kStream | kBin)
+        CASE(kSRD | kEmbedded | kStream | kBin | kEnergy)
+        CASE(kSRD | kEmbedded | kStream | kBin | kSortOut)
+        CASE(kSRD | kEmbedded | kStream | kBin | kEnergy | kSortOut)
+        CASE(kSRD | kThermo | kStream | kBin | kEnergy)
+        CASE(kSRD | kThermo | kStream | kBin | kEnergy | kSortOut)
+        CASE_F32(kSRD | kStream | kBin | kFixed)
+        CASE_F32(kSRD | kStream | kBin | kEnergy | kFixed)
+        CASE_F32(kSRD | kStream | kBin | kSortOut | kFixed)
+        CASE_F32(kSRD | kStream | kBin | kEnergy | kSortOut | kFixed)
+        CASE_F32(kSRD | kThermo | kStream | kBin | kEnergy | kFixed)
+        CASE_F32(kSRD | kThermo | kStream | kBin | kEnergy | kSortOut | kFixed)
+#undef CASE
+#undef CASE_F32
+        default: return fail(h, MPCD_EINVAL, "internal: brick pass combination not instantiated%s");
+    }
+    LAUNCH_CHECK(h);
+    return MPCD_OK;
+}
+
 int pass(mpcd_t *h, unsigned F, const PassPlan &pl)
 {
     const bool collide = (F & (kSRD | kATApply)) != 0, bin = (F & kBin) != 0;
     ProfScope prof(h, collide && bin ? ((F & kSortOut) ? MPCD_PROF_FUSED_SORT : MPCD_PROF_FUSED) : (collide ? MPCD_PROF_COLLIDE : (bin ? MPCD_PROF_BIN : MPCD_PROF_OTHER)));
+    if (h->brick_valid && (F & kSRD) && (F & kStream) && (F & kBin))   // the arrays are in brick order: one CTA per brick
+        return h->opt.precision == MPCD_FP64 ? launch_brick<double>(h, F, pl) : launch_brick<float>(h, F, pl);
     return h->opt.precision == MPCD_FP64 ? launch_pass<double>(h, F, pl) : launch_pass<float>(h, F, pl);
 }
 
@@ -322,9 +402,6 @@ int prepare(mpcd_t *h, int zset, bool sums, bool at, bool want_axes, uint64_t ax
 inline int zero_set(mpcd_t *h, int s, bool sums, bool at) { return prepare(h, s, sums, at, false, 0); }
 inline int ensure_axes(mpcd_t *h, uint64_t t) { return prepare(h, -1, false, false, true, t); }
 
-inline bool thermostatted(const mpcd_t *h) { return h->opt.thermostat != 0; }
-inline bool deterministic(const mpcd_t *h) { return h->opt.deterministic != 0; }
-inline unsigned fixed_flag(const mpcd_t *h) { return h->opt.deterministic != 0 ? kFixed : 0u; }
 
 // Maxwell-Boltzmann cell thermostat: xi of every cell from the complete sums (incl. energy) of step t in
 // set t & 1, into the 4th word of that step's axis sectors.
@@ -357,36 +434,43 @@ EmbArgs emb_args(mpcd_t *h, int cset, int bset, uint64_t step_collide, const dou
     return e;
 }
 
-// the beads' "streaming": md_substeps velocity-Verlet steps over one collision interval (PAPER.md:159)
-int emb_md(mpcd_t *h)
+MdArgs md_args(const mpcd_t *h)
 {
     MdArgs a{};
     a.pos = h->emb_pos; a.vel = h->emb_vel; a.chain_len = h->emb_chain_len; a.nsub = h->emb_nsub;
     a.k = h->emb_k; a.r0 = h->emb_r0; a.dt = h->opt.dt / h->emb_nsub;
     for (int d = 0; d < 3; ++d) a.L[d] = h->box[d];
-    ProfScope prof(h, MPCD_PROF_OTHER);
-    emb_md_verlet<<<(unsigned)(h->emb_n / h->emb_chain_len), kEmbThreads, (size_t)h->emb_chain_len * 10 * sizeof(double), h->stream>>>(a);
+    return a;
+}
+
+// one launch of the bead kernel (one block per chain) on stream st
+template <unsigned G> int emb_launch(mpcd_t *h, const EmbArgs &e, cudaStream_t st)
+{
+    ProfScope prof(h, MPCD_PROF_OTHER);              // (on the beads' own stream the pair of events on the handle's stream brackets nothing: the count is kept, the time is not)
+    emb_step<G><<<(unsigned)(h->emb_n / h->emb_chain_len), kEmbThreads, (size_t)h->emb_chain_len * 10 * sizeof(double), st>>>(md_args(h), e);
     LAUNCH_CHECK(h);
     return MPCD_OK;
+}
+
+// the beads' "streaming": md_substeps velocity-Verlet steps over one collision interval (PAPER.md:159)
+int emb_md(mpcd_t *h)
+{
+    const double zero[3] = {0, 0, 0};
+    return emb_launch<kEmbMd>(h, emb_args(h, 0, 0, 0, zero, 0.0), h->stream);
 }
 
 // bin the beads under `shift` and add them to the (zeroed) bead sums of set `bset`
 int emb_bin(mpcd_t *h, int bset, const double shift[3])
 {
-    ProfScope prof(h, MPCD_PROF_OTHER);
-    emb_bin_accumulate<<<grid_for(h->emb_n, kEmbThreads), kEmbThreads, 0, h->stream>>>(emb_args(h, bset, bset, 0, shift, 0.0));
-    LAUNCH_CHECK(h);
+    int rc = emb_launch<kEmbBinAcc>(h, emb_args(h, bset, bset, 0, shift, 0.0), h->stream);
     h->emb_zeroed[bset] = false;
-    return MPCD_OK;
+    return rc;
 }
 
 int emb_rotate(mpcd_t *h, int cset, uint64_t step_collide, double alpha)
 {
     const double zero[3] = {0, 0, 0};
-    ProfScope prof(h, MPCD_PROF_OTHER);
-    emb_collide<<<grid_for(h->emb_n, kEmbThreads), kEmbThreads, 0, h->stream>>>(emb_args(h, cset, cset, step_collide, zero, alpha));
-    LAUNCH_CHECK(h);
-    return MPCD_OK;
+    return emb_launch<kEmbRotate>(h, emb_args(h, cset, cset, step_collide, zero, alpha), h->stream);
 }
 
 // inside mpcd_step: [collide(step_collide) with set cset] + MD + [bin under `shift` into set bset] as one launch
@@ -398,16 +482,8 @@ template <unsigned G> int emb_step_launch(mpcd_t *h, int cset, int bset, uint64_
         CUDA_TRY(h, cudaEventRecord(h->emb_fork, h->stream));
         CUDA_TRY(h, cudaStreamWaitEvent(st, h->emb_fork, 0));
     }
-    MdArgs a{};
-    a.pos = h->emb_pos; a.vel = h->emb_vel; a.chain_len = h->emb_chain_len; a.nsub = h->emb_nsub;
-    a.k = h->emb_k; a.r0 = h->emb_r0; a.dt = h->opt.dt / h->emb_nsub;
-    for (int d = 0; d < 3; ++d) a.L[d] = h->box[d];
-    EmbArgs e = emb_args(h, cset, bset, step_collide, shift, alpha);
-    {
-        ProfScope prof(h, MPCD_PROF_OTHER);      // (with `beside` the pair of events on the handle's stream brackets nothing: the count is kept, the time is not)
-        emb_step<G><<<(unsigned)(h->emb_n / h->emb_chain_len), kEmbThreads, (size_t)h->emb_chain_len * 10 * sizeof(double), st>>>(a, e);
-        LAUNCH_CHECK(h);
-    }
+    int rc = emb_launch<G>(h, emb_args(h, cset, bset, step_collide, shift, alpha), st);
+    if (rc) return rc;
     if (st != h->stream) CUDA_TRY(h, cudaEventRecord(h->emb_join, st));
     if (G & kEmbBinAcc) h->emb_zeroed[bset] = false;
     return MPCD_OK;
@@ -420,23 +496,33 @@ int emb_join_stream(mpcd_t *h)
     return MPCD_OK;
 }
 
-// a8, first half: exclusive scan of the per-cell counts of accumulator set `s` -> cell_start (the write cursors)
+// a8, first half: exclusive scan of the per-cell counts of accumulator set `s` in sort-key order -> cell_start (the
+// write cursors) and, in brick-major order, the segment starts of the order being prepared (brick_start[bcur ^ 1])
 int scan_counts(mpcd_t *h, int s)
 {
-    const int ntiles = (int)((h->Nc + kScanTile - 1) / kScanTile);
+    const int ntiles = (int)((h->grid.nkeys + kScanTile - 1) / kScanTile);
     ProfScope prof(h, MPCD_PROF_SORT);
-    scan_tile_sums<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum, deterministic(h));
+    scan_tile_sums<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->grid, h->tile_sum, deterministic(h));
     LAUNCH_CHECK(h);
     scan_tile_offsets<<<1, 1024, 0, h->stream>>>(h->tile_sum, ntiles);
     LAUNCH_CHECK(h);
-    scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->Nc, h->tile_sum, h->cell_start, deterministic(h));
+    scan_cells<<<ntiles, kScanThreads, 0, h->stream>>>(h->acc[s], h->grid, h->tile_sum, h->cell_start, h->brick_start[h->bcur ^ 1], deterministic(h));
     LAUNCH_CHECK(h);
     return MPCD_OK;
 }
 
+// The particle arrays have just been written out in sort-key order of the bin of step t.
+void sorted_now(mpcd_t *h, uint64_t t)
+{
+    h->sorts += 1;
+    h->bcur ^= 1;
+    h->brick_valid = h->grid.on != 0;
+    shift_for(h, t, h->brick_shift);
+}
+
 // a8 as a pass of its own: counting sort by cell on the counts of accumulator set `s` (the cell of every particle is
 // cached in vel.w).  Inside mpcd_step the scatter is done by the next fused kernel instead (kSortOut).
-int do_sort(mpcd_t *h, int s)
+int do_sort(mpcd_t *h, int s, uint64_t t)
 {
     int rc = scan_counts(h, s);
     if (rc) return rc;
@@ -450,17 +536,11 @@ int do_sort(mpcd_t *h, int s)
         sort_scatter<float><<<grid_for(h->N, 256), 256, 0, h->stream>>>(make_args<float>(h, pl), h->cell_start, (float4 *)h->pos[dst], (float4 *)h->vel[dst], h->tag[dst]);
     LAUNCH_CHECK(h);
     h->pcur = dst;
-    h->sorts += 1;
+    sorted_now(h, t);
     return MPCD_OK;
 }
 
 inline bool sort_due(const mpcd_t *h, uint64_t t) { return h->opt.sort_period > 0 && (t % (uint64_t)h->opt.sort_period) == 0; }
-
-inline void shift_for(const mpcd_t *h, uint64_t step, double out[3])
-{
-    draw_shift(h, step, out);
-    if (h->opt.precision != MPCD_FP64) for (int d = 0; d < 3; ++d) out[d] = (double)(float)out[d];   // A5
-}
 
 // bin + accumulate (+ axes) for step t as a standalone block; energy always accumulated here
 int bin_accumulate(mpcd_t *h, uint64_t t)
@@ -474,6 +554,7 @@ int bin_accumulate(mpcd_t *h, uint64_t t)
     int rc = zero_set(h, set, true, false);
     if (rc) return rc;
     h->zeroed[set] = false;
+    h->xi_valid[set] = false;                         // the sums of this set are rewritten: its thermostat factors are stale
     rc = pass(h, kBin | kEnergy | fixed_flag(h), pl);
     if (rc) return rc;
     for (int d = 0; d < 3; ++d) h->shift_used[d] = pl.shift[d];
@@ -559,6 +640,7 @@ int mpcd_default_options(mpcd_options *opt)
     opt->sort_period = 25;
     opt->cell_energy = 1;
     opt->init_state = 1;
+    opt->brick = 1;
     return MPCD_OK;
 }
 
@@ -582,6 +664,7 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
     if (o.thermostat != 0 && o.thermostat != 1) return fail(nullptr, MPCD_EINVAL, "thermostat must be 0 or 1%s");
     if (o.deterministic != 0 && (o.deterministic != 1 || o.precision != MPCD_MIXED || o.rule != MPCD_SRD))
         return fail(nullptr, MPCD_EINVAL, "deterministic accumulation is 0 or 1 and needs the mixed model and the SRD rule%s");
+    if (o.brick != 0 && o.brick != 1) return fail(nullptr, MPCD_EINVAL, "brick must be 0 or 1%s");
     if (!(o.dt > 0) || o.sort_period < 0) return fail(nullptr, MPCD_EINVAL, "dt must be > 0 and sort_period >= 0%s");
     if ((o.alloc_fn == nullptr) != (o.free_fn == nullptr)) return fail(nullptr, MPCD_EINVAL, "alloc_fn and free_fn must be given together%s");
     int32_t n[3];
@@ -605,6 +688,16 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
     h->stream = static_cast<cudaStream_t>(o.stream);
     for (int d = 0; d < 3; ++d) { h->n[d] = n[d]; h->box[d] = box[d]; }
     h->Nc = (int64_t)n[0] * n[1] * n[2];
+    {   // the sort keys: brick-major when asked for and the key space (whole bricks) still fits int32, else the cell index
+        BrickGrid &g = h->grid;
+        double nkeys = (double)kBV;
+        for (int d = 0; d < 3; ++d) g.n[d] = n[d];
+        g.nb[0] = (n[0] + kBX - 1) / kBX; g.nb[1] = (n[1] + kBY - 1) / kBY; g.nb[2] = (n[2] + kBZ - 1) / kBZ;
+        for (int d = 0; d < 3; ++d) nkeys *= (double)g.nb[d];
+        g.on = (o.brick != 0 && nkeys < 2147483648.0) ? 1 : 0;
+        g.nkeys = g.on ? (int64_t)g.nb[0] * g.nb[1] * g.nb[2] * kBV : h->Nc;
+        h->nbricks = g.on ? g.nb[0] * g.nb[1] * g.nb[2] : 0;
+    }
     if (const char *e = std::getenv("MPCD_DEBUG_SYNC")) h->debug_sync = std::atoi(e) != 0;
     {
         int dev = 0, sms = 0;
@@ -623,7 +716,8 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
         if (!rc) rc = dev_alloc_t(h, &h->qacc[s], (size_t)h->Nc);
     }
     if (!rc) rc = dev_alloc_t(h, &h->cell_start, (size_t)h->Nc + 1);
-    if (!rc) rc = dev_alloc_t(h, &h->tile_sum, (size_t)((h->Nc + kScanTile - 1) / kScanTile) + 1);
+    if (!rc) rc = dev_alloc_t(h, &h->tile_sum, (size_t)((h->grid.nkeys + kScanTile - 1) / kScanTile) + 1);
+    for (int s = 0; s < 2 && !rc; ++s) rc = dev_alloc_t(h, &h->brick_start[s], (size_t)h->nbricks + 1);
     if (!rc) rc = dev_alloc_t(h, &h->d_max_occ, 64);
     if (!rc) rc = dev_alloc_t(h, &h->d_scalars, 32);
     if (!rc && o.rule == MPCD_AT) rc = ensure_at_buffers(h);
@@ -658,6 +752,7 @@ int mpcd_stream(mpcd_t *h)
     if (!rc && embedded(h)) rc = emb_md(h);          // the solute moves by MD over the same interval
     if (rc) return rc;
     h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false; h->emb_binned = false;
+    h->xi_valid[0] = h->xi_valid[1] = false;
     return MPCD_OK;
 }
 
@@ -717,7 +812,7 @@ int mpcd_sort(mpcd_t *h)
 {
     if (!h) return MPCD_EINVAL;
     if (!(h->bin_valid && h->counts_valid)) return fail(h, MPCD_ESTATE, "sort needs a valid bin (mpcd_shift_and_bin)%s");
-    return do_sort(h, h->ccur);
+    return do_sort(h, h->ccur, h->bin_step);
 }
 
 int mpcd_step(mpcd_t *h, int32_t nsteps)
@@ -744,6 +839,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;
     h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
+    h->xi_valid[set] = false;
     rc = pass(h, kStream | kBin | fe | fixed_flag(h) | (at ? (kATDraw | kATStored) : 0u), pl);   // AT: vel.xyz carries dv between the launches of this call
     if (!rc && emb) rc = emb_step_launch<kEmbMd | kEmbBinAcc>(h, set, set, t, pl.shift, h->opt.alpha);
     if (rc) return rc;
@@ -764,15 +860,16 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
         pl.cset = set; pl.bset = nxt;
         pl.step_collide = t; pl.step_bin = t + 1;
         h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
+        h->xi_valid[nxt] = false;
         rc = pass(h, (at ? (kATApply | kATDraw | kATStored) : (kSRD | ft | fb)) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
         if (rc) return rc;
         if (emb) { rc = emb_join_stream(h); if (rc) return rc; }
-        if (sort_pending) { h->pcur ^= 1; h->sorts += 1; }
+        if (sort_pending) { h->pcur ^= 1; sorted_now(h, t); }
         set = nxt; t += 1;
         if (ft) { rc = thermostat(h, t); if (rc) return rc; }
         sort_pending = sort_due(h, t);
     }
-    if (sort_pending) { rc = do_sort(h, set); if (rc) return rc; }
+    if (sort_pending) { rc = do_sort(h, set, t); if (rc) return rc; }
     // last collision
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;
@@ -820,7 +917,9 @@ int mpcd_set_state(mpcd_t *h, const void *pos4, const void *vel4, const uint32_t
     }
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     h->step = step;
-    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false;
+    h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false; h->emb_binned = false;
+    h->xi_valid[0] = h->xi_valid[1] = false;
+    h->brick_valid = false;                           // the caller's order is arbitrary
     return MPCD_OK;
 }
 
@@ -831,28 +930,30 @@ int mpcd_get_cells(mpcd_t *h, int32_t *count, double *sumv3, double *ke, double 
         return fail(h, MPCD_ESTATE, "cell sums are not valid: call mpcd_shift_and_bin first%s");
     if (axis3) { int rc0 = ensure_axes(h, h->bin_step); if (rc0) return rc0; }
     const size_t Nc = (size_t)h->Nc;
-    // stage through one temporary device buffer (SoA), sized for everything asked
-    const size_t bytes = Nc * (4 + 8 * (3 + 1 + 3 + 3 + 1));
-    void *tmp = nullptr;
-    cudaError_t e = cudaMalloc(&tmp, bytes);
-    if (e != cudaSuccess) { cudaGetLastError(); return fail(h, MPCD_ENOMEM, "cudaMalloc (get_cells staging): %s", cudaGetErrorString(e)); }
-    char *base = static_cast<char *>(tmp);
+    // stage through one device buffer (SoA) obtained from the handle's allocator on first use and kept
+    if (!h->cells_stage) {
+        int rc0 = dev_alloc(h, &h->cells_stage, Nc * (4 + 8 * (3 + 1 + 3 + 3 + 1)));
+        if (rc0) return rc0;
+    }
+    char *base = static_cast<char *>(h->cells_stage);
     double *d_sumv = reinterpret_cast<double *>(base);
     double *d_ke = d_sumv + 3 * Nc;
     double *d_u = d_ke + Nc;
     double *d_ax = d_u + 3 * Nc;
     double *d_kT = d_ax + 3 * Nc;
     int32_t *d_cnt = reinterpret_cast<int32_t *>(d_kT + Nc);
-    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->axis[h->bin_step & 1], h->Nc, h->m, deterministic(h), d_cnt, d_sumv, d_ke, d_u, d_ax, d_kT);
-    h->launches += 1;
-    int rc = MPCD_OK;
-    auto cp = [&](void *dst, const void *src, size_t b) {
-        if (dst && rc == MPCD_OK && cudaMemcpyAsync(dst, src, b, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) rc = fail(h, MPCD_ECUDA, "get_cells copy failed%s");
-    };
-    cp(count, d_cnt, Nc * 4); cp(sumv3, d_sumv, Nc * 24); cp(ke, d_ke, Nc * 8); cp(u3, d_u, Nc * 24); cp(axis3, d_ax, Nc * 24); cp(kTc, d_kT, Nc * 8);
-    if (cudaStreamSynchronize(h->stream) != cudaSuccess && rc == MPCD_OK) rc = fail(h, MPCD_ECUDA, "get_cells sync failed%s");
-    cudaFree(tmp);
-    return rc;
+    cell_unpack<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[h->ccur], h->qacc[h->ccur], h->axis[h->bin_step & 1], h->Nc, h->m, deterministic(h),
+                                                          count ? d_cnt : nullptr, sumv3 ? d_sumv : nullptr, ke ? d_ke : nullptr, u3 ? d_u : nullptr,
+                                                          axis3 ? d_ax : nullptr, kTc ? d_kT : nullptr);
+    LAUNCH_CHECK(h);
+    if (count) CUDA_TRY(h, cudaMemcpyAsync(count, d_cnt, Nc * 4, cudaMemcpyDeviceToHost, h->stream));
+    if (sumv3) CUDA_TRY(h, cudaMemcpyAsync(sumv3, d_sumv, Nc * 24, cudaMemcpyDeviceToHost, h->stream));
+    if (ke) CUDA_TRY(h, cudaMemcpyAsync(ke, d_ke, Nc * 8, cudaMemcpyDeviceToHost, h->stream));
+    if (u3) CUDA_TRY(h, cudaMemcpyAsync(u3, d_u, Nc * 24, cudaMemcpyDeviceToHost, h->stream));
+    if (axis3) CUDA_TRY(h, cudaMemcpyAsync(axis3, d_ax, Nc * 24, cudaMemcpyDeviceToHost, h->stream));
+    if (kTc) CUDA_TRY(h, cudaMemcpyAsync(kTc, d_kT, Nc * 8, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return MPCD_OK;
 }
 
 int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *vel3, const double *mass, int32_t chain_len, double k, double r0,
@@ -891,6 +992,7 @@ int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *v
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     h->emb_n = nb; h->emb_chain_len = chain_len; h->emb_nsub = md_substeps; h->emb_k = k; h->emb_r0 = r0;
     h->bin_valid = false; h->sums_valid = false; h->energy_valid = false; h->counts_valid = false; h->emb_binned = false;
+    h->xi_valid[0] = h->xi_valid[1] = false;
     return MPCD_OK;
 }
 
@@ -966,6 +1068,7 @@ int mpcd_get_stats(mpcd_t *h, mpcd_stats *out)
         CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     }
     out->max_occupancy = h->max_occ;
+    if (h->grid.on) { out->brick[0] = kBX; out->brick[1] = kBY; out->brick[2] = kBZ; out->brick[3] = kH; }
     out->step = h->step; out->kernel_launches = h->launches; out->sorts = h->sorts; out->device_bytes = h->device_bytes;
     return MPCD_OK;
 }

@@ -220,6 +220,23 @@ template <typename T> __device__ __forceinline__ int bin_axis(T x, T s, T inv_a,
     return i;
 }
 
+// Alg. 1 lines 5-12: v' = u + xi R(alpha, n)(v - u), in double, with the contractions spelled out so
+// that every kernel that collides a particle produces the same bits (opt.deterministic relies on it).
+__device__ __forceinline__ void srd_rotate(double vx, double vy, double vz, double ux, double uy, double uz, double nx, double ny, double nz,
+                                           double xi, double cos_a, double sin_a, double &ox, double &oy, double &oz)
+{
+    const double wx = vx - ux, wy = vy - uy, wz = vz - uz;                                      // lines 5-6
+    const double ndw = __fma_rn(nz, wz, __fma_rn(ny, wy, __dmul_rn(nx, wx)));                   // line 7
+    const double omc = 1.0 - cos_a;
+    const double cx = __fma_rn(ny, wz, -__dmul_rn(nz, wy)), cy = __fma_rn(nz, wx, -__dmul_rn(nx, wz)), cz = __fma_rn(nx, wy, -__dmul_rn(ny, wx));
+    const double rx = __fma_rn(__dmul_rn(nx, ndw), omc, __fma_rn(cx, sin_a, __dmul_rn(wx, cos_a)));
+    const double ry = __fma_rn(__dmul_rn(ny, ndw), omc, __fma_rn(cy, sin_a, __dmul_rn(wy, cos_a)));
+    const double rz = __fma_rn(__dmul_rn(nz, ndw), omc, __fma_rn(cz, sin_a, __dmul_rn(wz, cos_a)));
+    ox = __fma_rn(rx, xi, ux); oy = __fma_rn(ry, xi, uy); oz = __fma_rn(rz, xi, uz);            // lines 8-12
+}
+__device__ __forceinline__ double sq_norm(double x, double y, double z) { return __fma_rn(z, z, __fma_rn(y, y, __dmul_rn(x, x))); }
+
+
 // ---------------------------------------------------------------------------------------
 // Warp-level machinery of the per-particle pass.
 //
@@ -301,7 +318,7 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
     const int lane = threadIdx.x & 31;
     const double dx0 = (double)fx, dy0 = (double)fy, dz0 = (double)fz;
     A vx = Ops::from(dx0), vy = Ops::from(dy0), vz = Ops::from(dz0);
-    A q = kEnergy ? Ops::from(dx0 * dx0 + dy0 * dy0 + dz0 * dz0) : A(0);
+    A q = kEnergy ? Ops::from(sq_norm(dx0, dy0, dz0)) : A(0);
     unsigned peers = __match_any_sync(full, c);
     const int size = __popc(peers);
     const int rank0 = __popc(peers & ((1u << lane) - 1u));
@@ -318,7 +335,7 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
         if (next && alive) {
             const double dx = (double)tx, dy = (double)ty, dz = (double)tz;
             vx += Ops::from(dx); vy += Ops::from(dy); vz += Ops::from(dz);
-            if (kEnergy) q += Ops::from(dx * dx + dy * dy + dz * dz);
+            if (kEnergy) q += Ops::from(sq_norm(dx, dy, dz));
             if (kExtra) { ex += ux; ey += uy; ez += uz; }
         }
         rounds = 1;
@@ -391,5 +408,57 @@ template <int K> __device__ __forceinline__ void block_sum_to_global(double (&v)
     }
     __syncthreads();
 }
+
+// ---------------------------------------------------------------------------------------
+// Brick-major order of the sort and the tiles of the brick kernel (mpcd_brick.cuh).
+// ---------------------------------------------------------------------------------------
+#ifndef MPCD_BRICK_X
+#define MPCD_BRICK_X 4
+#endif
+#ifndef MPCD_BRICK_Y
+#define MPCD_BRICK_Y 4
+#endif
+#ifndef MPCD_BRICK_Z
+#define MPCD_BRICK_Z 4
+#endif
+#ifndef MPCD_BRICK_HALO
+#define MPCD_BRICK_HALO 2
+#endif
+constexpr int kBX = MPCD_BRICK_X, kBY = MPCD_BRICK_Y, kBZ = MPCD_BRICK_Z, kBV = kBX * kBY * kBZ;
+constexpr int kH = MPCD_BRICK_HALO;
+constexpr int kWX = kBX + kH, kWY = kBY + kH, kWZ = kBZ + kH, kW = kWX * kWY * kWZ;
+
+// floor(n / d) for 0 <= n < 2^31 and a run-time invariant d >= 1: (n m) >> (31 + s), s = ceil(log2 d), m = ceil(2^(31+s) / d)
+// (Granlund & Montgomery's round-up multiplier for 31-bit dividends: m < 2^32, the product fits 64 bits).
+struct Div31 { uint32_t m, s; };
+inline Div31 make_div31(uint32_t d)
+{
+    uint32_t s = 0;
+    while (((uint64_t)1 << s) < d) ++s;
+    const uint64_t two = (uint64_t)1 << (31 + s);
+    return Div31{(uint32_t)((two + d - 1) / d), s};
+}
+__device__ __forceinline__ uint32_t div31(uint32_t n, const Div31 &dv) { return (uint32_t)(((uint64_t)n * dv.m) >> (31 + dv.s)); }
+
+// The sort key.  Linear order (on == 0): key = cell index.  Brick-major order: key = brick * kBV + cell inside the brick,
+// bricks x-fastest over nb = ceil(n / kB) per axis, cells x-fastest inside the brick; keys of cells outside the box
+// (ragged last bricks) are holes with count 0.
+struct BrickGrid {
+    int32_t on;
+    int32_t n[3], nb[3];
+    int64_t nkeys;
+};
+__host__ __device__ __forceinline__ int64_t key_to_cell(int64_t k, const BrickGrid &g)       // -1 for a hole
+{
+    if (!g.on) return k;
+    const int64_t b = k / kBV;
+    const int l = (int)(k - b * kBV);
+    const int lx = l % kBX, ly = (l / kBX) % kBY, lz = l / (kBX * kBY);
+    const int bx = (int)(b % g.nb[0]), by = (int)((b / g.nb[0]) % g.nb[1]), bz = (int)(b / ((int64_t)g.nb[0] * g.nb[1]));
+    const int ix = bx * kBX + lx, iy = by * kBY + ly, iz = bz * kBZ + lz;
+    if (ix >= g.n[0] || iy >= g.n[1] || iz >= g.n[2]) return -1;
+    return ix + (int64_t)g.n[0] * (iy + (int64_t)g.n[1] * iz);
+}
+
 
 }  // namespace mpcdk

@@ -42,59 +42,6 @@ struct MdArgs {
     double k, r0, dt, L[3];
 };
 
-// Velocity Verlet between two collisions, nsub steps of length dt: one block per chain with the
-// chain's state in shared memory ([x, v, f: 3 doubles each][mass] per bead = 80 B), threads strided over the beads.
-__global__ void __launch_bounds__(kEmbThreads) emb_md_verlet(const MdArgs a)
-{
-    extern __shared__ double sm[];
-    const int n = a.chain_len;
-    double *sx = sm, *sv = sm + 3 * n, *sf = sm + 6 * n, *smass = sm + 9 * n;
-    const int64_t base = (int64_t)blockIdx.x * n;
-    const double L[3] = {a.L[0], a.L[1], a.L[2]};
-    for (int j = threadIdx.x; j < n; j += kEmbThreads) {
-        const double4 p = ld_d4(a.pos + base + j), v = ld_d4(a.vel + base + j);
-        sx[3 * j] = p.x; sx[3 * j + 1] = p.y; sx[3 * j + 2] = p.z; smass[j] = p.w;
-        sv[3 * j] = v.x; sv[3 * j + 1] = v.y; sv[3 * j + 2] = v.z;
-    }
-    __syncthreads();
-    auto forces = [&]() {                                // reads sx of the neighbours, writes this thread's sf
-        for (int j = threadIdx.x; j < n; j += kEmbThreads) {
-            double d[3], g, fx = 0.0, fy = 0.0, fz = 0.0;
-            if (j > 0) { bond(sx + 3 * (j - 1), sx + 3 * j, L, a.k, a.r0, d, g); fx = g * d[0]; fy = g * d[1]; fz = g * d[2]; }
-            if (j + 1 < n) { bond(sx + 3 * j, sx + 3 * (j + 1), L, a.k, a.r0, d, g); fx -= g * d[0]; fy -= g * d[1]; fz -= g * d[2]; }
-            sf[3 * j] = fx; sf[3 * j + 1] = fy; sf[3 * j + 2] = fz;
-        }
-    };
-    forces();
-    for (int s = 0; s < a.nsub; ++s) {
-        __syncthreads();                                 // every force has been computed from the old positions
-        for (int j = threadIdx.x; j < n; j += kEmbThreads) {
-            const double h = 0.5 * a.dt / smass[j];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                sv[3 * j + c] += h * sf[3 * j + c];
-                double x = sx[3 * j + c] + sv[3 * j + c] * a.dt;
-                if (x < 0.0) x += L[c];
-                if (x >= L[c]) x -= L[c];
-                sx[3 * j + c] = x;
-            }
-        }
-        __syncthreads();
-        forces();
-        for (int j = threadIdx.x; j < n; j += kEmbThreads) {
-            const double h = 0.5 * a.dt / smass[j];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) sv[3 * j + c] += h * sf[3 * j + c];
-        }
-    }
-    for (int j = threadIdx.x; j < n; j += kEmbThreads) {
-        double4 v = ld_d4(a.vel + base + j);             // keeps .w (the cached cell index)
-        v.x = sv[3 * j]; v.y = sv[3 * j + 1]; v.z = sv[3 * j + 2];
-        st_d4(a.pos + base + j, double4{sx[3 * j], sx[3 * j + 1], sx[3 * j + 2], smass[j]});
-        st_d4(a.vel + base + j, v);
-    }
-}
-
 struct EmbArgs {
     double4 *pos, *vel;
     int64_t nb;
@@ -104,53 +51,23 @@ struct EmbArgs {
     double shift[3], inv_a, mass_solvent, cos_a, sin_a;
 };
 
-// Bin the beads under the step's grid shift (the same expression as the solvent's, in double; A6) and add their
-// momentum and mass to their cells ("including the solute particles in ... cell property calculation").
-__global__ void __launch_bounds__(kEmbThreads) emb_bin_accumulate(const EmbArgs a)
-{
-    const int64_t i = (int64_t)blockIdx.x * kEmbThreads + threadIdx.x;
-    if (i >= a.nb) return;
-    const double4 p = ld_d4(a.pos + i);
-    double4 v = ld_d4(a.vel + i);
-    const int ix = bin_axis<double>(p.x, a.shift[0], a.inv_a, a.n[0]);
-    const int iy = bin_axis<double>(p.y, a.shift[1], a.inv_a, a.n[1]);
-    const int iz = bin_axis<double>(p.z, a.shift[2], a.inv_a, a.n[2]);
-    const int c = ix + a.n[0] * (iy + a.n[1] * iz);
-    v.w = __longlong_as_double((long long)c);
-    st_d4(a.vel + i, v);
-    double *e = a.eacc + 4 * (size_t)c;
-    atomicAdd(e, p.w * v.x); atomicAdd(e + 1, p.w * v.y); atomicAdd(e + 2, p.w * v.z); atomicAdd(e + 3, p.w);
-}
-
 // Mass-weighted mean velocity of a cell holding solvent sums s = {S, N} and bead sums e = {P, M} (A10).
 __device__ __forceinline__ void embedded_mean(const f64x4 &s, const f64x4 &e, double m, double &ux, double &uy, double &uz)
 {
-    const double inv = __drcp_rn(m * s.w + e.w);
-    ux = (m * s.x + e.x) * inv; uy = (m * s.y + e.y) * inv; uz = (m * s.z + e.z) * inv;
+    const double inv = __drcp_rn(__fma_rn(m, s.w, e.w));     // contractions spelled out: every kernel forms the same bits
+    ux = __dmul_rn(__fma_rn(m, s.x, e.x), inv); uy = __dmul_rn(__fma_rn(m, s.y, e.y), inv); uz = __dmul_rn(__fma_rn(m, s.z, e.z), inv);
 }
 
-// SRD rotation of the beads (eq. 2, Alg. 1) about their cell's axis, relative to the mass-weighted cell mean.
-__global__ void __launch_bounds__(kEmbThreads) emb_collide(const EmbArgs a)
-{
-    const int64_t i = (int64_t)blockIdx.x * kEmbThreads + threadIdx.x;
-    if (i >= a.nb) return;
-    double4 v = ld_d4(a.vel + i);
-    const size_t c = (size_t)__double_as_longlong(v.w);
-    const f64x4 s = ld256(a.sums + 4 * c), e = ld256(a.esum + 4 * c), n = ld256(a.axis + 4 * c);
-    double ux, uy, uz;
-    embedded_mean(s, e, a.mass_solvent, ux, uy, uz);
-    const double wx = v.x - ux, wy = v.y - uy, wz = v.z - uz;
-    const double ndw = n.x * wx + n.y * wy + n.z * wz, omc = 1.0 - a.cos_a;
-    v.x = ux + (wx * a.cos_a + (n.y * wz - n.z * wy) * a.sin_a + n.x * ndw * omc);
-    v.y = uy + (wy * a.cos_a + (n.z * wx - n.x * wz) * a.sin_a + n.y * ndw * omc);
-    v.z = uz + (wz * a.cos_a + (n.x * wy - n.y * wx) * a.sin_a + n.z * ndw * omc);
-    st_d4(a.vel + i, v);
-}
-
-// The three bead kernels of one step inside mpcd_step as ONE launch (config 5 is half launch-bound: 5 M solvent
-// particles take 0.12 ms per step): per chain block, collide the beads with the complete sums of step t (kRotate), advance
-// them by MD over the next interval (kMd), then bin them under the shift of step t + 1 and add them to that step's
-// bead sums (kBinAcc).  The same arithmetic, in the same order, as emb_collide, emb_md_verlet and emb_bin_accumulate.
+// The bead kernel, one block per chain with the chain's state in shared memory ([x, v, f: 3 doubles each][mass] per
+// bead = 80 B), any combination of:
+//   kEmbRotate  SRD rotation of the beads (eq. 2, Alg. 1) about their cell's axis, relative to the mass-weighted mean
+//   kEmbMd      velocity Verlet between two collisions, nsub steps of length dt
+//   kEmbBinAcc  bin the beads under the step's grid shift (the solvent's expression, in double; A6) and add their
+//               momentum and mass to their cells ("including the solute particles in ... cell property
+//               calculation")
+// Inside mpcd_step all three are ONE launch (config 5 is half launch-bound: 5 M solvent particles take 0.12 ms per
+// step): collide with the complete sums of step t, MD over the next interval, bin under the shift of step t + 1.  The
+// unfused ABI calls launch the single-flag instantiations.
 enum : unsigned { kEmbRotate = 1u, kEmbMd = 2u, kEmbBinAcc = 4u };
 
 template <unsigned G>
@@ -169,11 +86,7 @@ __global__ void __launch_bounds__(kEmbThreads) emb_step(const MdArgs a, const Em
             const f64x4 s = ld256(e.sums + 4 * c), b = ld256(e.esum + 4 * c), ax = ld256(e.axis + 4 * c);
             double ux, uy, uz;
             embedded_mean(s, b, e.mass_solvent, ux, uy, uz);
-            const double wx = v.x - ux, wy = v.y - uy, wz = v.z - uz;
-            const double ndw = ax.x * wx + ax.y * wy + ax.z * wz, omc = 1.0 - e.cos_a;
-            v.x = ux + (wx * e.cos_a + (ax.y * wz - ax.z * wy) * e.sin_a + ax.x * ndw * omc);
-            v.y = uy + (wy * e.cos_a + (ax.z * wx - ax.x * wz) * e.sin_a + ax.y * ndw * omc);
-            v.z = uz + (wz * e.cos_a + (ax.x * wy - ax.y * wx) * e.sin_a + ax.z * ndw * omc);
+            srd_rotate(v.x, v.y, v.z, ux, uy, uz, ax.x, ax.y, ax.z, 1.0, e.cos_a, e.sin_a, v.x, v.y, v.z);
         }
         sx[3 * j] = p.x; sx[3 * j + 1] = p.y; sx[3 * j + 2] = p.z; smass[j] = p.w;
         sv[3 * j] = v.x; sv[3 * j + 1] = v.y; sv[3 * j + 2] = v.z;

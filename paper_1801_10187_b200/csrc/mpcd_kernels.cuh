@@ -126,16 +126,11 @@ __global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_
                 embedded_mean(s, ld256_nc(a.esum + 4 * (size_t)c), a.mass, ux, uy, uz);
             } else {
                 const double inv = __drcp_rn(s.w);               // N_c >= 1: this particle is a member
-                ux = s.x * inv; uy = s.y * inv; uz = s.z * inv;
+                ux = __dmul_rn(s.x, inv); uy = __dmul_rn(s.y, inv); uz = __dmul_rn(s.z, inv);
             }
-            const double wx = (double)v.x - ux, wy = (double)v.y - uy, wz = (double)v.z - uz;   // lines 5-6
-            const double ndw = n.x * wx + n.y * wy + n.z * wz;                                  // line 7
-            const double omc = 1.0 - a.cos_a;
-            const double rx = wx * a.cos_a + (n.y * wz - n.z * wy) * a.sin_a + n.x * ndw * omc;
-            const double ry = wy * a.cos_a + (n.z * wx - n.x * wz) * a.sin_a + n.y * ndw * omc;
-            const double rz = wz * a.cos_a + (n.x * wy - n.y * wx) * a.sin_a + n.z * ndw * omc;
-            const double xi = (F & kThermo) ? n.w : 1.0;                                        // lines 8-10
-            v.x = (T)(ux + rx * xi); v.y = (T)(uy + ry * xi); v.z = (T)(uz + rz * xi);           // lines 11-12
+            double ox, oy, oz;                                   // lines 5-12
+            srd_rotate((double)v.x, (double)v.y, (double)v.z, ux, uy, uz, n.x, n.y, n.z, (F & kThermo) ? n.w : 1.0, a.cos_a, a.sin_a, ox, oy, oz);
+            v.x = (T)ox; v.y = (T)oy; v.z = (T)oz;
         }
     }
     if (F & kATApply) {
@@ -233,9 +228,12 @@ __global__ void __launch_bounds__(256) cell_thermostat(const double *acc, const 
     const int n = (int)s.w;
     double xi = 1.0;
     if (n >= 2) {
-        const double erel = 0.5 * m * (acc_value(qacc[c], fixed) - (s.x * s.x + s.y * s.y + s.z * s.z) / s.w);
+        // E_rel = KE - M_c u^2 / 2 (A12) cancels when the cell drifts much faster than it is warm: below 1e-9 of the cell's
+        // kinetic energy the difference is rounding noise of the fp64 sums, and the cell is left alone like E_k = 0 (A26)
+        const double q = acc_value(qacc[c], fixed);
+        const double erel = 0.5 * m * (q - (s.x * s.x + s.y * s.y + s.z * s.z) / s.w);
         const double ehat = draw_cell_energy(seed, step, (uint32_t)c, n, kT);
-        if (erel > 0.0) xi = sqrt(ehat / erel);
+        if (erel > 1e-9 * 0.5 * m * q) xi = sqrt(ehat / erel);
     }
     axis[4 * c + 3] = xi;
 }
@@ -306,14 +304,23 @@ __global__ void __launch_bounds__(256) cell_unpack(const double *acc, const doub
 // ---------------------------------------------------------------------------------------
 constexpr int kScanThreads = 256, kScanItems = 16, kScanTile = kScanThreads * kScanItems;
 
-__global__ void __launch_bounds__(kScanThreads) scan_tile_sums(const double *acc, int64_t Nc, int32_t *tile_sum, bool fixed)
+// The scan runs over SORT KEYS (mpcd_device.cuh: the cell index, or the brick-major key); count of a key = count of its
+// cell, 0 for a hole.  cell_start stays indexed by the cell; brick_start[b] (brick-major order only) = first slot of
+// brick b, brick_start[number of bricks] = N.
+__device__ __forceinline__ int key_count(const double *acc, int64_t key, const BrickGrid &g, bool fixed, int64_t &cell)
+{
+    cell = key < g.nkeys ? key_to_cell(key, g) : -1;
+    return cell >= 0 ? (int)acc_count(acc[4 * cell + 3], fixed) : 0;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_tile_sums(const double *acc, const BrickGrid g, int32_t *tile_sum, bool fixed)
 {
     __shared__ int sm[kScanThreads / 32];
     const int64_t base = (int64_t)blockIdx.x * kScanTile;
     int s = 0;
     for (int k = 0; k < kScanItems; ++k) {
-        const int64_t c = base + (int64_t)k * kScanThreads + threadIdx.x;
-        if (c < Nc) s += (int)acc_count(acc[4 * c + 3], fixed);
+        int64_t c;
+        s += key_count(acc, base + (int64_t)k * kScanThreads + threadIdx.x, g, fixed, c);
     }
     s = __reduce_add_sync(0xffffffffu, s);
     if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
@@ -351,15 +358,17 @@ __global__ void __launch_bounds__(1024) scan_tile_offsets(int32_t *tile_sum, int
     }
 }
 
-__global__ void __launch_bounds__(kScanThreads) scan_cells(const double *acc, int64_t Nc, const int32_t *tile_off, int32_t *cell_start, bool fixed)
+__global__ void __launch_bounds__(kScanThreads) scan_cells(const double *acc, const BrickGrid g, const int32_t *tile_off, int32_t *cell_start,
+                                                           int32_t *brick_start, bool fixed)
 {
-    // thread t owns kScanItems consecutive cells of the tile
+    // thread t owns kScanItems consecutive keys of the tile
     __shared__ int sm[kScanThreads];
     const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
     int x[kScanItems];
+    int64_t cell[kScanItems];
     int s = 0;
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) { x[k] = (base + k < Nc) ? (int)acc_count(acc[4 * (base + k) + 3], fixed) : 0; s += x[k]; }
+    for (int k = 0; k < kScanItems; ++k) { x[k] = key_count(acc, base + k, g, fixed, cell[k]); s += x[k]; }
     sm[threadIdx.x] = s;
     __syncthreads();
     for (int o = 1; o < kScanThreads; o <<= 1) {
@@ -370,7 +379,12 @@ __global__ void __launch_bounds__(kScanThreads) scan_cells(const double *acc, in
     }
     int run = tile_off[blockIdx.x] + sm[threadIdx.x] - s;
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) { if (base + k < Nc) cell_start[base + k] = run; run += x[k]; }
+    for (int k = 0; k < kScanItems; ++k) {
+        if (cell[k] >= 0) cell_start[cell[k]] = run;
+        if (g.on && base + k < g.nkeys && (base + k) % kBV == 0) brick_start[(base + k) / kBV] = run;
+        run += x[k];
+        if (g.on && base + k == g.nkeys - 1) brick_start[g.nkeys / kBV] = run;
+    }
 }
 
 template <typename T>
