@@ -34,7 +34,8 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_1801_10187_b200 import replicas, synth  # noqa: E402
+import workloads as synth  # noqa: E402
+from paper_1801_10187_b200 import replicas  # noqa: E402
 
 METRIC = "mpcd_particle_steps_per_s"
 UNIT = "particle-steps/s"

@@ -83,12 +83,13 @@ typedef struct mpcd_options {
                               fixed-point integers (40 fractional bits), so the trajectory is bit-reproducible whatever the order of
                               warps, atomics and particles in memory; results stay within the mixed-model tolerance of the fp64
                               sums.  Mixed model + SRD rule only (MPCD_EINVAL otherwise; no embedded beads); default 0 */
-    int32_t brick;         /* 1 (default): the sort (sect. 3.8) orders the particles BRICK-major -- cells grouped in bricks of
+    int32_t brick;         /* 1: the sort (sect. 3.8) orders the particles BRICK-major -- cells grouped in bricks of
                               brick[0] x brick[1] x brick[2] cells (mpcd_stats.brick; compile-time), bricks x-fastest over
                               ceil(n_d / brick[d]) per axis, cells x-fastest inside a brick -- and mpcd_step runs its steady-state kernel
                               with one thread block per brick and the cell side of the step in shared memory.  The
                               order inside the sort is free (A20): results are the same up to fp64 summation order.
-                              0: ascending cell index and the warp-level kernel */
+                              0 (default): ascending cell index and the warp-level kernel (the faster of the two on the north-star workload,
+                              DESIGN.md 5.1) */
     void *stream;          /* cudaStream_t the library enqueues on; NULL = the legacy default stream */
     mpcd_alloc_fn alloc_fn;
     mpcd_free_fn free_fn;

@@ -33,7 +33,11 @@
  * one-collision thermalisation (test_oracle_thermostat.py); embedded solute: the
  * velocity-Verlet dimer against its closed form, forces vs numerical gradients, MD
  * momentum / bounded energy, mass-weighted collision invariants, equipartition
- * (test_oracle_embedded.py).
+ * (test_oracle_embedded.py); initial condition oracle_init_*: A23 restated per particle from the
+ * pinned Philox words, KS tests, zero net momentum; the rotation sense inside
+ * oracle_collide_srd_beads against scipy's Rotation; oracle_collide_srd_xi bit-identical to
+ * oracle_collide_srd at xi = 1 and doubling the relative velocity at xi = 2
+ * (test_oracle_pins_r2.py).
  * parity unpinned: none.
  */
 #include <math.h>

@@ -141,7 +141,7 @@ class MPCD:
 
     def __init__(self, box, N, a=1.0, m=1.0, kT=1.0, seed=0, *, precision="mixed", rule="srd", dt=0.1,
                  alpha=math.radians(130.0), sort_period=25, cell_energy=True, init_state=True, thermostat=False, deterministic=False,
-                 brick=True, device="cuda:0", use_torch_allocator=True, stream=None):
+                 brick=False, device="cuda:0", use_torch_allocator=True, stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1801_10187_b200 needs a CUDA device (no CPU fallback)")

@@ -314,25 +314,39 @@ BrickArgs brick_args(const mpcd_t *h, const PassPlan &pl)
     }
     g.div_nx = make_div31((uint32_t)h->n[0]);
     g.div_nxy = make_div31((uint32_t)h->n[0] * (uint32_t)h->n[1]);
+    g.div_nbx = make_div31((uint32_t)h->grid.nb[0]);
+    g.div_nbxy = make_div31((uint32_t)h->grid.nb[0] * (uint32_t)h->grid.nb[1]);
     int e = 0;
     std::frexp(h->sigma, &e);                        // unit = 2^e >= sqrt(kT / m)
     if (deterministic(h)) {
-        g.sv = g.sq = kFixScale; g.inv_sv = g.inv_sq = kFixInv; g.vmax = HUGE_VAL;
+        g.sv = kFixScale; g.inv_sv = g.inv_sq = kFixInv; g.qrel = 1.0; g.vmax = HUGE_VAL;
     } else {
         g.sv = std::ldexp(1.0, 48 - e); g.inv_sv = std::ldexp(1.0, e - 48);
-        g.sq = std::ldexp(1.0, 44 - 2 * e); g.inv_sq = std::ldexp(1.0, 2 * e - 44);
+        g.inv_sq = std::ldexp(1.0, 2 * e - 44); g.qrel = std::ldexp(1.0, -4 - e);
         g.vmax = std::ldexp(8.0, e);
     }
     return g;
+}
+
+template <typename T, unsigned F> int launch_brick_t(mpcd_t *h, const PassArgs<T> &a, const BrickArgs &g)
+{
+    static bool configured = false;                  // dynamic shared memory above 48 KB is opt-in, once per instantiation
+    if (!configured) {
+        CUDA_TRY(h, cudaFuncSetAttribute(brick_pass<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BrickSmem<F>::bytes));
+        configured = true;
+    }
+    brick_pass<T, F><<<(unsigned)h->nbricks, kBrickThreads, BrickSmem<F>::bytes, h->stream>>>(a, g);
+    return MPCD_OK;
 }
 
 template <typename T> int launch_brick(mpcd_t *h, unsigned F, const PassPlan &pl)
 {
     const PassArgs<T> a = make_args<T>(h, pl);
     const BrickArgs g = brick_args(h, pl);
+    int rc = MPCD_OK;
     switch (F) {
-#define CASE(f) case (f): brick_pass<T, (f)><<<(unsigned)h->nbricks, kBrickThreads, 0, h->stream>>>(a, g); break;
-#define CASE_F32(f) case (f): if constexpr (sizeof(T) == 4) { brick_pass<T, (f)><<<(unsigned)h->nbricks, kBrickThreads, 0, h->stream>>>(a, g); break; } else return fail(h, MPCD_EINVAL, "internal: fixed-point sums need the mixed model%s");
+#define CASE(f) case (f): rc = launch_brick_t<T, (f)>(h, a, g); break;
+#define CASE_F32(f) case (f): if constexpr (sizeof(T) == 4) { rc = launch_brick_t<T, (f)>(h, a, g); break; } else return fail(h, MPCD_EINVAL, "internal: fixed-point sums need the mixed model%s");
         CASE(kSRD | kStream | kBin)
         CASE(kSRD | kStream | kBin | kEnergy)
         CASE(kSRD | kStream | kBin | kSortOut)
@@ -353,6 +367,7 @@ template <typename T> int launch_brick(mpcd_t *h, unsigned F, const PassPlan &pl
 #undef CASE_F32
         default: return fail(h, MPCD_EINVAL, "internal: brick pass combination not instantiated%s");
     }
+    if (rc) return rc;
     LAUNCH_CHECK(h);
     return MPCD_OK;
 }
@@ -640,7 +655,7 @@ int mpcd_default_options(mpcd_options *opt)
     opt->sort_period = 25;
     opt->cell_energy = 1;
     opt->init_state = 1;
-    opt->brick = 1;
+    opt->brick = 0;
     return MPCD_OK;
 }
 
@@ -1115,7 +1130,7 @@ int mpcd_abi_version(void) { return MPCD_ABI_VERSION; }
 
 const char *mpcd_build_info(void)
 {
-    return "mpcd-b200 ABI 2, sm_100a, nvcc " __VERSION__
+    return "mpcd-b200 ABI 3, sm_100a, nvcc " __VERSION__
 #ifdef __CUDACC_VER_MAJOR__
            " / CUDA"
 #endif

@@ -48,8 +48,9 @@ struct BrickArgs {
     const int32_t *brick_start;    // first array slot of every brick's segment, nbricks + 1 entries
     int32_t nb[3];
     int32_t og[3], oa[3];          // window origin minus the brick's first cell, per axis: step collided / step binned
-    Div31 div_nx, div_nxy;
-    double sv, inv_sv, sq, inv_sq; // fixed-point scales of the shared-memory partial sums (velocity, |v|^2) and their inverses
+    Div31 div_nx, div_nxy, div_nbx, div_nbxy;
+    double sv, inv_sv, inv_sq;     // fixed-point scale of the shared-memory partial sums of the velocities and the inverse scales (velocity, |v|^2)
+    double qrel;                   // scale of |v|^2 over scale of the velocities (a power of two: applied before the lanes rotate their values)
     double vmax;                   // |v_d| below this fits the headroom
 };
 
@@ -59,30 +60,64 @@ __device__ __forceinline__ void smem_add64(unsigned *lo, unsigned *hi, long long
 {
     const unsigned vl = (unsigned)(unsigned long long)v, vh = (unsigned)((unsigned long long)v >> 32);
     const unsigned old = atomicAdd(lo, vl);
-    atomicAdd(hi, vh + ((unsigned)(old + vl) < old ? 1u : 0u));
+    unsigned vhc;                                       // high word + carry of (old + vl)
+    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %3, 0;\n\t}" : "=r"(vhc) : "r"(old), "r"(vl), "r"(vh));
+    atomicAdd(hi, vhc);
 }
 
-__device__ __forceinline__ int pmod(int v, int n) { int r = v % n; return r < 0 ? r + n : r; }
+// v mod n for a v that is at most a few n outside [0, n) (no integer division)
+__device__ __forceinline__ int wrap(int v, int n)
+{
+    while (v < 0) v += n;
+    while (v >= n) v -= n;
+    return v;
+}
 
+// Shared memory of one CTA (dynamic: bricks larger than 4 x 4 x 4 need more than the static 48 KB).
+template <unsigned F> struct BrickSmem {
+    static constexpr int NV = (F & kEnergy) ? 4 : 3;            // fixed-point sums per cell: Sx, Sy, Sz [, sum |v|^2]
+    static constexpr int NA = (F & kThermo) ? 4 : 3;            // axis [, xi]
+    static constexpr size_t bytes = (size_t)kW * (8 * (3 + NA) + 4 * (2 * NV + 2));
+};
+
+// Thread -> particle mapping.  A warp's 32 lanes are four QUARTERS of 8 lanes; quarter k of the CTA streams through its
+// own contiguous sub-segment of the brick, 8 consecutive particles (one full 128-byte line of float4) per iteration.
+// The loads stay whole-line accesses, but the lanes of one ATOMS / LDS instruction now come from four places ~4 cells
+// apart instead of 32 consecutive particles of ~3 cells, so fewer lanes of an instruction hit the same window cell
+// (same-address shared-memory atomics serialise: 6.3 wavefronts per ATOMS with the consecutive mapping, ncu).
 template <typename T, unsigned F>
 __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pass(const PassArgs<T> a, const BrickArgs g)
 {
     using V4 = typename Vec4<T>::type;
     static_assert((F & kSRD) && (F & kStream) && (F & kBin), "the brick kernel is the fused steady-state SRD step");
     constexpr bool kE = (F & kEnergy) != 0, kFx = (F & kFixed) != 0, kTh = (F & kThermo) != 0, kEm = (F & kEmbedded) != 0, kSo = (F & kSortOut) != 0;
-    constexpr int NV = kE ? 4 : 3;
+    constexpr int NV = BrickSmem<F>::NV, NA = BrickSmem<F>::NA;
     using Ops = AccOps<typename std::conditional<kFx, long long, double>::type>;
-    __shared__ double sU[3][kW];                        // window of the step collided: mean velocity
-    __shared__ double sA[kTh ? 4 : 3][kW];              // ... axis (and the thermostat's xi)
-    __shared__ unsigned sLo[NV][kW], sHi[NV][kW], sCnt[kW];   // window of the step binned: fixed-point partial sums
+    extern __shared__ __align__(16) unsigned char brick_smem[];
+    double (*sU)[kW] = reinterpret_cast<double (*)[kW]>(brick_smem);                 // [3][kW]  window of the step collided: mean velocity
+    double (*sA)[kW] = sU + 3;                                                       // [NA][kW] ... axis (and the thermostat's xi)
+    unsigned (*sLo)[kW] = reinterpret_cast<unsigned (*)[kW]>(sA + NA);               // [NV][kW] window of the step binned: fixed-point partial sums
+    unsigned (*sHi)[kW] = sLo + NV;                                                  // [NV][kW]
+    unsigned *sCnt = reinterpret_cast<unsigned *>(sHi + NV);                         // [kW]
+    int *sCell = reinterpret_cast<int *>(sCnt + kW);                                 // [kW]     global cell of every slot of that window
     const int tid = threadIdx.x;
     const int b = blockIdx.x;
     const int lo = g.brick_start[b], hi = g.brick_start[b + 1];
     if (lo >= hi) return;                               // empty brick
     const int n0 = a.n[0], n1 = a.n[1], n2 = a.n[2];
-    const int bx = b % g.nb[0], by = (b / g.nb[0]) % g.nb[1], bz = b / (g.nb[0] * g.nb[1]);
-    const int gx0 = pmod(bx * kBX + g.og[0], n0), gy0 = pmod(by * kBY + g.og[1], n1), gz0 = pmod(bz * kBZ + g.og[2], n2);
-    const int ax0 = pmod(bx * kBX + g.oa[0], n0), ay0 = pmod(by * kBY + g.oa[1], n1), az0 = pmod(bz * kBZ + g.oa[2], n2);
+    const int bz = (int)div31((uint32_t)b, g.div_nbxy), br = b - bz * g.nb[0] * g.nb[1];
+    const int by = (int)div31((uint32_t)br, g.div_nbx), bx = br - by * g.nb[0];
+    const int gx0 = wrap(bx * kBX + g.og[0], n0), gy0 = wrap(by * kBY + g.og[1], n1), gz0 = wrap(bz * kBZ + g.og[2], n2);
+    const int ax0 = wrap(bx * kBX + g.oa[0], n0), ay0 = wrap(by * kBY + g.oa[1], n1), az0 = wrap(bz * kBZ + g.oa[2], n2);
+
+    // quarter k streams blocks [k m, (k + 1) m) of 8 particles, counted from the 128-byte line the segment starts in
+    const int a0 = lo & ~7;
+    const int nblk = (hi - a0 + 7) >> 3;
+    const int m = (nblk + kBrickThreads / 8 - 1) / (kBrickThreads / 8);
+    int i = a0 + 8 * (tid >> 3) * m + (tid & 7);
+    auto clamped = [&](int idx) { return idx < lo ? lo : (idx >= hi ? hi - 1 : idx); };
+    V4 vn = load4(a.vel + clamped(i));                  // the first block's loads are in flight while the window is built
+    V4 pn = load4(a.pos + clamped(i));
 
     // 1. window build
     for (int w = tid; w < kW; w += kBrickThreads) {
@@ -105,10 +140,15 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
         }
         sU[0][w] = ux; sU[1][w] = uy; sU[2][w] = uz;
         sA[0][w] = n.x; sA[1][w] = n.y; sA[2][w] = n.z;
-        if (kTh) sA[kTh ? 3 : 0][w] = n.w;
+        if (kTh) sA[NA - 1][w] = n.w;
 #pragma unroll
         for (int k = 0; k < NV; ++k) { sLo[k][w] = 0u; sHi[k][w] = 0u; }
         sCnt[w] = 0u;
+        cx = ax0 + lx; cy = ay0 + ly; cz = az0 + lz;
+        while (cx >= n0) cx -= n0;
+        while (cy >= n1) cy -= n1;
+        while (cz >= n2) cz -= n2;
+        sCell[w] = cx + n0 * (cy + n1 * cz);
     }
     __syncthreads();
 
@@ -119,12 +159,7 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
             const int w = idx >> 2, k = idx & 3;
             const unsigned cnt = sCnt[w];
             if (cnt == 0u) continue;
-            const int lx = w % kWX, ly = (w / kWX) % kWY, lz = w / (kWX * kWY);
-            int cx = ax0 + lx, cy = ay0 + ly, cz = az0 + lz;
-            while (cx >= n0) cx -= n0;
-            while (cy >= n1) cy -= n1;
-            while (cz >= n2) cz -= n2;
-            const size_t c = (size_t)cx + (size_t)n0 * ((size_t)cy + (size_t)n1 * (size_t)cz);
+            const size_t c = (size_t)sCell[w];
             if (k < 3) {
                 const long long x = (long long)(((unsigned long long)sHi[k][w] << 32) | sLo[k][w]);
                 Ops::red(a.acc + 4 * c + k, kFx ? fixed_bits(x) : (double)x * g.inv_sv);
@@ -140,8 +175,10 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
 
     // 2. the particles of this brick's segment
     const uint32_t nxy = (uint32_t)n0 * (uint32_t)n1;
+    const int rot = (tid & 7) % NV;                      // which value this lane adds first, and where the others go
+    const int off0 = rot * kW, off1 = ((rot + 1) % NV) * kW, off2 = ((rot + 2) % NV) * kW, off3 = ((rot + 3) % NV) * kW;
     int since = 0;
-    for (int base = lo; base < hi; base += kBrickThreads) {
+    for (int j = 0; j < m; ++j, i += 8) {
         if (since + kBrickThreads > kFlushLimit) {
             __syncthreads();
             flush();
@@ -155,13 +192,14 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
             since = 0;
         }
         since += kBrickThreads;
-        const int i = base + tid;
-        const bool valid = i < hi;
-        const int il = valid ? i : hi - 1;               // lanes past the end work on a copy of the last particle and store nothing
-        V4 v = load4(a.vel + il);
-        V4 p = load4(a.pos + il);
+        const bool valid = i >= lo && i < hi;            // other lanes work on a copy of a particle of the segment and store nothing
+        V4 v = vn, p = pn;
+        if (j + 1 < m) {                                 // the next block's loads fly during this block's arithmetic
+            vn = load4(a.vel + clamped(i + 8));
+            pn = load4(a.pos + clamped(i + 8));
+        }
         uint32_t tag = 0;
-        if (kSo) tag = a.tag[il];
+        if (kSo) tag = a.tag[clamped(i)];
         const int c = w_to_cell(v.w);                    // cell of the step being collided
         int64_t o = i;
         if (kSo && valid) o = atomicAdd(a.cursor + c, 1);
@@ -177,7 +215,7 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
                 const int w = lx + kWX * (ly + kWY * lz);
                 ux = sU[0][w]; uy = sU[1][w]; uz = sU[2][w];
                 nx = sA[0][w]; ny = sA[1][w]; nz = sA[2][w];
-                if (kTh) xi = sA[kTh ? 3 : 0][w];
+                if (kTh) xi = sA[NA - 1][w];
             } else {                                     // drifted out of the window: the round-1 gather
                 f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);
                 const f64x4 n = ld256_nc(a.axis + 4 * (size_t)c);
@@ -188,8 +226,11 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
                     const double inv = __drcp_rn(s.w);
                     ux = __dmul_rn(s.x, inv); uy = __dmul_rn(s.y, inv); uz = __dmul_rn(s.z, inv);
                 }
-                nx = n.x; ny = n.y; nz = n.z;
-                if (kTh) xi = n.w;
+                // consume the loaded axis INSIDE this rare branch: a register first read after the branches merge would make
+                // every warp wait there on the scoreboard slot these loads share with the prefetch of the next block (ncu:
+                // 25 % of all samples on that one instruction)
+                nx = __dadd_rn(n.x, 0.0); ny = __dadd_rn(n.y, 0.0); nz = __dadd_rn(n.z, 0.0);
+                if (kTh) xi = __dadd_rn(n.w, 0.0);
             }
             double ox, oy, oz;
             srd_rotate((double)v.x, (double)v.y, (double)v.z, ux, uy, uz, nx, ny, nz, xi, a.cos_a, a.sin_a, ox, oy, oz);
@@ -213,13 +254,28 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
             if (lx < 0) lx += n0;
             if (ly < 0) ly += n1;
             if (lz < 0) lz += n2;
-            const bool fits = kFx || (fabs(dx) < g.vmax && fabs(dy) < g.vmax && fabs(dz) < g.vmax);
+            const T vmax = (T)g.vmax;
+            const bool fits = kFx || (fabs(v.x) < vmax && fabs(v.y) < vmax && fabs(v.z) < vmax);
             if (lx < kWX && ly < kWY && lz < kWZ && fits) {
                 const int w = lx + kWX * (ly + kWY * lz);
-                smem_add64(&sLo[0][w], &sHi[0][w], kFx ? to_fixed(dx) : __double2ll_rn(dx * g.sv));
-                smem_add64(&sLo[1][w], &sHi[1][w], kFx ? to_fixed(dy) : __double2ll_rn(dy * g.sv));
-                smem_add64(&sLo[2][w], &sHi[2][w], kFx ? to_fixed(dz) : __double2ll_rn(dz * g.sv));
-                if (kE) smem_add64(&sLo[NV - 1][w], &sHi[NV - 1][w], kFx ? to_fixed(q) : __double2ll_rn(q * g.sq));
+                // Lanes of one instruction that share a window cell would serialise on its address (shared-memory atomics do
+                // not merge; ncu: 4.8 wavefronts per ATOMS): lane l therefore starts with value (l mod NV), so that in any one
+                // ATOMS the lanes of a cell are spread over the NV per-value arrays (3.3).  The rotation is two conditional swaps
+                // of the doubles; |v|^2 is first brought to the velocities' scale (a power of two: exact) so that one multiply
+                // serves whatever value a slot holds.
+                double y0 = dx, y1 = dy, y2 = dz, y3 = kFx ? q : q * g.qrel;
+                if (NV == 4) {
+                    if (rot & 1) { const double t = y0; y0 = y1; y1 = y2; y2 = y3; y3 = t; }
+                    if (rot & 2) { double t = y0; y0 = y2; y2 = t; t = y1; y1 = y3; y3 = t; }
+                } else {
+                    if (rot >= 1) { const double t = y0; y0 = y1; y1 = y2; y2 = t; }
+                    if (rot >= 2) { const double t = y0; y0 = y1; y1 = y2; y2 = t; }
+                }
+                unsigned *plo = &sLo[0][w], *phi = &sHi[0][w];
+                smem_add64(plo + off0, phi + off0, kFx ? to_fixed(y0) : __double2ll_rn(y0 * g.sv));
+                smem_add64(plo + off1, phi + off1, kFx ? to_fixed(y1) : __double2ll_rn(y1 * g.sv));
+                smem_add64(plo + off2, phi + off2, kFx ? to_fixed(y2) : __double2ll_rn(y2 * g.sv));
+                if (NV == 4) smem_add64(plo + off3, phi + off3, kFx ? to_fixed(y3) : __double2ll_rn(y3 * g.sv));
                 atomicAdd(&sCnt[w], 1u);
             } else {                                     // outside the window (or too fast for the headroom): straight to the global sums
                 double *s = a.acc + 4 * (size_t)cn;

@@ -41,11 +41,11 @@ def test_north_star_entry_points_present(lib):
 
 def test_abi_version_and_defaults(lib):
     from paper_1801_10187_b200.binding import Options
-    assert lib.mpcd_abi_version() == 2
+    assert lib.mpcd_abi_version() == 3
     assert b"sm_100a" in lib.mpcd_build_info()
     o = Options()
     assert lib.mpcd_default_options(C.byref(o)) == 0
-    assert o.precision == 0 and o.rule == 0 and o.sort_period == 25 and o.cell_energy == 1
+    assert o.precision == 0 and o.rule == 0 and o.sort_period == 25 and o.cell_energy == 1 and o.brick == 0
     assert abs(o.dt - 0.1) < 1e-15 and abs(o.alpha - 130 * 3.141592653589793 / 180) < 1e-15
     assert lib.mpcd_default_options(None) == -1
 

@@ -3,7 +3,7 @@ sort, repeated mpcd_step calls landing on and off sort steps, zero-copy device p
 import numpy as np
 import pytest
 
-from paper_1801_10187_b200 import synth
+import workloads as synth
 
 pytestmark = pytest.mark.gpu
 

@@ -6,7 +6,7 @@ import math
 import numpy as np
 import pytest
 
-from paper_1801_10187_b200 import synth
+import workloads as synth
 
 pytestmark = pytest.mark.gpu
 K, R0, NSUB, MB = 1000.0, 0.5, 10, 5.0

@@ -10,7 +10,7 @@ PAPER.md:45)."""
 import numpy as np
 import pytest
 
-from paper_1801_10187_b200 import synth
+import workloads as synth
 
 pytestmark = pytest.mark.gpu
 

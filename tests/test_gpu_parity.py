@@ -7,7 +7,7 @@ import math
 import numpy as np
 import pytest
 
-from paper_1801_10187_b200 import synth
+import workloads as synth
 
 pytestmark = pytest.mark.gpu
 
@@ -33,6 +33,18 @@ def _pair(oracle, n, M, seed, dtype, a=1.0, m=1.0, kT=1.0, N=None, **kw):
 
 def _tol(dtype, sigma=1.0):
     return (FP64_TOL if dtype == np.float64 else MIXED_TOL) * sigma
+
+
+def _sort_key(cell, n, brick):
+    """The sort key include/mpcd.h documents for mpcd_sort: the cell index, or the brick-major key."""
+    if brick[0] == 0:
+        return cell.astype(np.int64)
+    B = np.array(brick[:3], dtype=np.int64)
+    nb = (np.array(n, dtype=np.int64) + B - 1) // B
+    c = cell.astype(np.int64)
+    ix, iy, iz = c % n[0], (c // n[0]) % n[1], c // (n[0] * n[1])
+    b = ((iz // B[2]) * nb[1] + iy // B[1]) * nb[0] + ix // B[0]
+    return b * B.prod() + ((iz % B[2]) * B[1] + iy % B[1]) * B[0] + ix % B[0]
 
 
 def _by_tag(state):
@@ -128,14 +140,15 @@ def test_calls_out_of_order_return_estate(oracle):
         g.collide_srd(1.0)          # the sums are stale after a collision
 
 
+@pytest.mark.parametrize("brick", [True, False])
 @pytest.mark.parametrize("dtype", [np.float32, np.float64])
-def test_sort_keeps_the_multiset_and_orders_by_cell(oracle, dtype):
-    g, o = _pair(oracle, (9, 6, 11), 10, 23, dtype)
+def test_sort_keeps_the_multiset_and_orders_by_cell(oracle, dtype, brick):
+    g, o = _pair(oracle, (9, 6, 11), 10, 23, dtype, brick=brick)
     g.stream(); g.shift_and_bin()
     before = g.get_state()
     g.sort()
     after = g.get_state()
-    assert np.all(np.diff(after["cell"]) >= 0)                              # cell[] non-decreasing
+    assert np.all(np.diff(_sort_key(after["cell"], g.n, g.stats()["brick"])) >= 0)   # ascending sort key (include/mpcd.h, mpcd_sort)
     a, b = _by_tag(after), _by_tag(before)
     for k in ("tag", "pos", "vel", "cell"):
         assert np.array_equal(a[k], b[k]), k                                 # multiset unchanged bit for bit

@@ -9,7 +9,7 @@ import pytest
 from scipy import stats
 from scipy.spatial.transform import Rotation
 
-from paper_1801_10187_b200 import synth
+import workloads as synth
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 FORMS = json.load(open(os.path.join(HERE, "golden", "closed_forms.json")))["cases"]

@@ -9,7 +9,7 @@ import math
 import numpy as np
 import pytest
 
-from paper_1801_10187_b200 import synth
+import workloads as synth
 
 
 def test_velocity_verlet_dimer_closed_form_and_minimum_image(oracle):

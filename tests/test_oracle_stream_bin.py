@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 from scipy import stats
 
-from paper_1801_10187_b200 import synth
+import workloads as synth
 
 
 @pytest.mark.parametrize("dtype", [np.float32, np.float64])

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 from scipy import stats
 
-from paper_1801_10187_b200 import synth
+import workloads as synth
 
 
 @pytest.mark.parametrize("n", [2, 3, 10, 31])

@@ -1,4 +1,5 @@
-"""Seeded synthetic inputs shared by the tests, bench.py and smoke().
+"""Seeded synthetic inputs shared by the tests, bench.py and smoke() -- a module of its own, outside both the product
+package and the oracle.
 
 Holds none of the method's arithmetic: only numpy's own generators producing the
 paper's workload recipe: positions i.i.d. uniform in the box,
