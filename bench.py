@@ -11,8 +11,14 @@ particles, mixed precision) -- the configuration the north-star target is quoted
 seeded and synthetic (paper recipe) and far larger than L2 (6.4 GB of particle
 state vs 126 MB), so no L2 flush is needed between iterations.
 
+Timing protocol ("whole multiples of the sort period so the sort is amortised in"; the sort and
+its period are PAPER.md:173, :177-179): the untimed warm-up runs at least --warmup steps and ends on a step
+with t % sort_period == 0; the timed region is ONE mpcd_step call of ceil(--steps / sort_period) * sort_period
+steps, so it always contains one sort per period whatever --steps says.  The line reports both counts
+(`steps` = timed, `steps_requested`, `warmup` = requested, `warmup_run`) and `check.sorts_in_timed_region`.
+
 Prints ONE JSON line (rank 0).  `value` = particle-steps/s with the state resident in HBM, timed
-with CUDA events on the library's stream around mpcd_step(K), max over ranks.  `e2e` = the same
+with CUDA events on the library's stream around that mpcd_step call, max over ranks.  `e2e` = the same
 metric through the C ABI with HOST buffers: every step copies the state from pinned host memory
 (mpcd_set_state), steps, and copies it back (mpcd_get_state).  `roofline` = algorithmic bytes of
 the steady-state fused kernel / its live-measured duration, against the measured HBM copy peak.
@@ -58,23 +64,44 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(workload: str, precision: str):
-    """DRAM bytes per launch of the fused kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the
-    committed `ncu --set full` summary profiles/ncu_traffic.csv (workload,precision,bytes,source), if any."""
+def csrc_hash() -> str:
+    """sha256 (first 16 hex digits) over the kernel sources, in name order: what an ncu capture is stamped with."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_1801_10187_b200", "csrc")
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(name.encode())
+            with open(os.path.join(d, name), "rb") as f:
+                h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload: str, precision: str, brick: int):
+    """DRAM bytes per launch of the step kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
+    `ncu --set full` summary profiles/ncu_traffic.csv (workload,precision,brick,bytes,csrc_hash,source).  A capture is
+    only quoted for the kernel sources it was taken on: returns (bytes or None, note)."""
+    found = None
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
             for line in f:
                 w = [x.strip() for x in line.split(",")]
-                if len(w) >= 3 and w[0] == workload and w[1] == precision:
-                    return float(w[2])
+                if len(w) >= 5 and w[0] == workload and w[1] == precision and w[2] == str(int(brick)):
+                    found = (float(w[3]), w[4])
     except Exception:
         pass
-    return None
+    if found is None:
+        return None, "no ncu capture committed for this workload"
+    if found[1] != csrc_hash():
+        return None, f"ncu capture is of kernel sources {found[1]}, the tree is {csrc_hash()}: not quoted"
+    return found[0], f"ncu --set full capture of kernel sources {found[1]} (profiles/ncu_traffic.csv)"
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi clocks / throttle reasons DURING the GPU arm (B200_PROFILING.md recipe), sampled every 10 ms from
+    before the warm-up to after the per-kernel timing leg (all of it back-to-back GPU work around the timed region).
+    `sm_mhz` is the median over the samples taken under load (utilization.gpu >= 50 %)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,utilization.gpu,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
@@ -84,8 +111,11 @@ class ClockSampler:
         try:
             fd, self.path = tempfile.mkstemp(suffix=".csv")
             os.close(fd)
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20"],
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "10"],
                                          stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+            t0 = time.time()                      # the first sample arrives once nvidia-smi has attached to the device
+            while time.time() - t0 < 3.0 and os.path.getsize(self.path) == 0:
+                time.sleep(0.01)
         except Exception:
             self.proc = None
         return self
@@ -99,17 +129,17 @@ class ClockSampler:
                 self.proc.kill()
 
     def summary(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "samples_under_load": 0}
         if not self.path:
             return out
-        sm, mx, reasons, power = [], [], set(), []
+        rows, reasons = [], set()
         try:
             for line in open(self.path):
                 f = [x.strip() for x in line.split(",")]
                 if len(f) < 9:
                     continue
                 try:
-                    sm.append(float(f[1])); mx.append(float(f[2])); power.append(float(f[3]))
+                    rows.append((float(f[1]), float(f[2]), float(f[3]), float(f[4])))
                 except ValueError:
                     continue
                 for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
@@ -118,13 +148,14 @@ class ClockSampler:
             os.unlink(self.path)
         except Exception:
             pass
-        if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm),
-                       power_w_max=float(max(power)))
+        if rows:
+            load = [r for r in rows if r[3] >= 50.0] or rows
+            out.update(sm_mhz=float(np.median([r[0] for r in load])), sm_max_mhz=float(max(r[1] for r in rows)), reasons=sorted(reasons),
+                       samples=len(rows), samples_under_load=len([r for r in rows if r[3] >= 50.0]), power_w_max=float(max(r[2] for r in rows)))
         return out
 
 
-def oracle_sample(cfg, precision, steps, warmup, n_sample):
+def oracle_sample(cfg, precision, steps, warmup, n_sample, barrier=None):
     """The oracle, as it stands, on a bounded sample of the workload: the same recipe (density, rule,
     parameters, sort period) in a smaller box.  Returns (particle-steps/s, seconds per step, N)."""
     from oracle import oracle as O
@@ -140,11 +171,49 @@ def oracle_sample(cfg, precision, steps, warmup, n_sample):
         o.set_embedded(bp, bv, bm, ch["chain_len"], ch["k"], ch["r0"], ch["md_substeps"])
     for _ in range(warmup):
         o.step()
+    if barrier is not None:
+        barrier.wait()
     t0 = time.perf_counter()
     for _ in range(steps):
         o.step()
     dt = time.perf_counter() - t0
     return pos.shape[0] * steps / dt, dt / steps, pos.shape[0]
+
+
+def _oracle_worker(cfg, precision, steps, warmup, n_sample, seed_offset, barrier, queue):
+    """One process of the all-core timing: its own box (own seed), the oracle as it stands; all processes leave the
+    barrier together, so the boxes are stepped at the same time and share the host's memory bandwidth."""
+    cfg = dict(cfg, seed=cfg["seed"] + seed_offset)
+    try:
+        queue.put(oracle_sample(cfg, precision, steps, warmup, n_sample, barrier=barrier))
+    except Exception as e:                                   # a worker that dies must not hang the others at the barrier
+        try:
+            barrier.abort()
+        except Exception:
+            pass
+        queue.put(("error", repr(e), 0))
+
+
+def oracle_all_cores(cfg, precision, steps, warmup, n_sample):
+    """The oracle on ALL host cores (SURVEY.md 8d "Oracle timing beside it" (b); the paper's own CPU runs are one MPI rank
+    per core, each with its own sub-domain): one process per core, each stepping an independent
+    sub-box of the workload -- the unmodified single-threaded oracle, replicated, with no communication at all, which is
+    an upper bound for a domain-decomposed CPU run.  Returns (aggregate particle-steps/s, cores, particles per process)."""
+    import multiprocessing as mp
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    ctx = mp.get_context("spawn")                            # never fork a process that holds a CUDA context
+    barrier, queue = ctx.Barrier(cores), ctx.Queue()
+    procs = [ctx.Process(target=_oracle_worker, args=(cfg, precision, steps, warmup, n_sample, 1000 + k, barrier, queue)) for k in range(cores)]
+    for p in procs:
+        p.start()
+    res = [queue.get() for _ in procs]
+    for p in procs:
+        p.join()
+    bad = [r for r in res if r[0] == "error"]
+    if bad:
+        raise RuntimeError(f"all-core oracle timing failed: {bad[0][1]}")
+    slowest = max(r[1] for r in res)                         # seconds per step of the slowest process
+    return sum(r[2] for r in res) / slowest, cores, res[0][2]
 
 
 def sample_box(cfg, target_particles):
@@ -198,6 +267,7 @@ def main():
     ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
     ap.add_argument("--cell-energy", type=int, default=1)
     ap.add_argument("--sort-period", type=int, default=25)
+    ap.add_argument("--brick", type=int, default=0, help="1: brick-major sort order + the brick-tiled step kernel")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -209,8 +279,6 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.warmup < 3:
-        args.warmup = 3
 
     if args.impl == "reference":
         return run_reference(args, cfg, rank, world)
@@ -236,101 +304,114 @@ def main():
     pos, vel, tag = synth.solvent(n, M, seed=seed, dtype=dtype)
     N = pos.shape[0]
     sim = MPCD([float(x) for x in n], N, seed=seed, precision=args.precision, rule=cfg["rule"], sort_period=args.sort_period,
-               cell_energy=bool(args.cell_energy), init_state=False, device=f"cuda:{local_rank}")
+               cell_energy=bool(args.cell_energy), init_state=False, brick=bool(args.brick), device=f"cuda:{local_rank}")
     sim.set_state(pos, vel, tag)
     if "chains" in cfg:
         ch = cfg["chains"]
         bp, bv, bm = synth.chains(n, ch["n_chains"], ch["chain_len"], seed=seed + 1, mass=ch["mass"], r0=ch["r0"])
         sim.set_embedded(bp, bv, bm, ch["chain_len"], ch["k"], ch["r0"], ch["md_substeps"])
 
-    # ---- device-resident throughput ----
-    sim.step(args.warmup)
-    barrier()
-    l0 = sim.stats()["kernel_launches"]
+    # ---- device-resident throughput: whole sort periods, starting on a sort step ----
+    P = max(args.sort_period, 0)
+    up = (lambda x: -(-x // P) * P) if P > 0 else (lambda x: x)
+    warm_run, timed = up(max(args.warmup, 1)), up(max(args.steps, 1))
+    if warm_run < 3:
+        raise SystemExit("bench.py: at least 3 warm-up steps are required (timing rules); give --warmup >= 3")
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local_rank) as clocks:
+        sim.step(warm_run)                                    # ends on t % P == 0: the timed call starts with a sort step
+        barrier()
+        st0 = sim.stats()
         barrier()
         ev0.record()
-        sim.step(args.steps)
+        sim.step(timed)
         ev1.record()
         barrier()
-    ms = ev0.elapsed_time(ev1)
-    launches = sim.stats()["kernel_launches"] - l0
-    value, ms_max = replicas.whole_job_throughput(float(N) * args.steps, ms, dist if world > 1 else None, dev)
+        ms = ev0.elapsed_time(ev1)
+        st1 = sim.stats()
+        # ---- per-kernel durations, live, CUDA events on the library's stream, over one more whole sort period ----
+        sim.set_profiling(True)
+        sim.step(max(P, 1) + 1)
+        prof = sim.get_profile()
+        sim.set_profiling(False)
+    launches = st1["kernel_launches"] - st0["kernel_launches"]
+    sorts_timed = st1["sorts"] - st0["sorts"]
+    value, ms_max = replicas.whole_job_throughput(float(N) * timed, ms, dist if world > 1 else None, dev)
 
-    # ---- per-kernel durations, live, CUDA events on the library's stream ----
-    sim.set_profiling(True)
-    sim.step(max(args.sort_period, 1) + 1)
-    prof = sim.get_profile()
-    sim.set_profiling(False)
     fused_ms = prof["fused"][0] / max(prof["fused"][1], 1)
     per_step_ms = {k: (v[0] / max(v[1], 1), v[1]) for k, v in prof.items() if v[1]}
     peak, peak_src = measured_peak()
     algo = algorithmic_bytes_per_particle(args.precision, M) * N
     achieved = algo / (fused_ms * 1e-3) / 1e9 if fused_ms > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "particle_pass<collide+stream+bin+accumulate> (steady-state fused step)",
+    traffic, traffic_note = ncu_traffic(args.config, args.precision, args.brick)
+    kernel = "brick_pass" if args.brick else "particle_pass"
+    roofline = {"bound": "hbm", "kernel": f"{kernel}<collide+stream+bin+accumulate> (steady-state fused step)",
                 "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": ncu_traffic(args.config, args.precision), "algorithmic_bytes_per_launch": algo,
-                "kernel_ms": fused_ms, "kernel_share_of_step": fused_ms / (ms_max / args.steps),
+                "traffic": traffic, "traffic_source": traffic_note, "algorithmic_bytes_per_launch": algo,
+                "kernel_ms": fused_ms, "kernel_share_of_step": fused_ms / (ms_max / timed),
                 "stage_ms_per_launch": {k: round(v[0], 4) for k, v in per_step_ms.items()},
-                "whole_step_frac": algo / (ms_max / args.steps * 1e-3) / 1e9 / peak}
+                "whole_step_frac": algo / (ms_max / timed * 1e-3) / 1e9 / peak}
 
     # ---- end to end through the C ABI with host buffers ----
     e2e = None
     if not args.no_e2e:
         st = sim.get_state(cell=False)
-        hp = torch.from_numpy(st["pos"]).pin_memory()
-        hv = torch.from_numpy(st["vel"]).pin_memory()
-        ht = torch.from_numpy(st["tag"].view(np.int32)).pin_memory()
-        out = {"pos": torch.empty_like(hp).pin_memory(), "vel": torch.empty_like(hv).pin_memory()}
+        bufs = []
+        for _ in range(2):                                    # two sets of pinned host buffers: a step's output set is the next step's input set
+            bufs.append({"pos": torch.empty((N, 4), dtype=torch.float32 if dtype == np.float32 else torch.float64).pin_memory(),
+                         "vel": torch.empty((N, 4), dtype=torch.float32 if dtype == np.float32 else torch.float64).pin_memory(),
+                         "tag": torch.empty(N, dtype=torch.int32).pin_memory()})
+        bufs[0]["pos"].copy_(torch.from_numpy(st["pos"])); bufs[0]["vel"].copy_(torch.from_numpy(st["vel"]))
+        bufs[0]["tag"].copy_(torch.from_numpy(st["tag"].view(np.int32)))
         step0 = st["step"]
         del st
 
         def one(k):
-            sim.set_state(hp, hv, ht, step=step0 + k)         # H2D from pinned host memory
+            src, dst = bufs[k & 1], bufs[(k & 1) ^ 1]
+            sim.set_state(src["pos"], src["vel"], src["tag"], step=step0 + k)   # H2D from pinned host memory
             sim.step(1)
-            sim.get_state(out=out)                            # D2H of the step's result
-            hp.copy_(out["pos"]); hv.copy_(out["vel"])        # the next step's input is this step's output
+            sim.get_state(out=dst)                                              # D2H of the step's result (tags travel: a sort step permutes them)
         one(0)
         barrier()
         t0 = time.perf_counter()
-        ev0.record()
         for k in range(args.e2e_steps):
             one(1 + k)
-        ev1.record()
         barrier()
         wall = time.perf_counter() - t0
         t = torch.tensor([wall], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        nbytes = int(sum(x.numel() * x.element_size() for x in bufs[0].values()))
         e2e = {"value": world * N * args.e2e_steps / float(t.item()), "unit": UNIT,
-               "h2d_bytes_per_step": int(hp.numel() * hp.element_size() + hv.numel() * hv.element_size() + ht.numel() * 4),
-               "d2h_bytes_per_step": int(hp.numel() * hp.element_size() + hv.numel() * hv.element_size()),
+               "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                "steps": args.e2e_steps, "ms_per_step": float(t.item()) / args.e2e_steps * 1e3,
-               "note": "mpcd_set_state(pinned host) + mpcd_step(1) + mpcd_get_state(pinned host) per step; includes a host-side copy of the result into the next input"}
-        del hp, hv, ht, out
+               "note": "mpcd_set_state(pinned host) + mpcd_step(1) + mpcd_get_state(pinned host) per step; the output buffers of a step are the input buffers of the next"}
+        del bufs
 
-    P, KE, kT = sim.get_thermo()
+    Pm, KE, kT = sim.get_thermo()
     stats = sim.stats()
     sim.close()
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n_sample = sample_box(cfg, args.cpu_particles)
-        v, sps, Ns = oracle_sample(cfg, args.precision, args.cpu_steps, 1, n_sample)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"{n_sample[0]}^3-cell sub-box of {args.config} at the same density ({Ns} particles), {args.cpu_steps} steps after 1 warm-up, "
-                         f"{sps * args.cpu_steps:.1f} s of CPU work; host has {os.cpu_count()} cores, the oracle is single-threaded"}
+        v1, sps, Ns = oracle_sample(cfg, args.precision, args.cpu_steps, 1, n_sample)
+        n_each = sample_box(cfg, max(args.cpu_particles // 4, 1))
+        vall, cores, Ne = oracle_all_cores(cfg, args.precision, args.cpu_steps, 1, n_each)
+        cpu = {"value": vall, "unit": UNIT, "cores": cores, "kind": "oracle", "single_thread": v1, "all_cores": vall,
+               "sample": f"single_thread: {n_sample[0]}^3-cell sub-box of {args.config} at the same density ({Ns} particles), {args.cpu_steps} steps after 1 warm-up, "
+                         f"{sps * args.cpu_steps:.1f} s of CPU work; all_cores: {cores} processes (one per host core), each the unmodified oracle on its own "
+                         f"{n_each[0]}^3-cell sub-box ({Ne} particles), {args.cpu_steps} steps started together, aggregate = particles of all boxes / slowest process's time per step"}
 
     if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": timed, "steps_requested": args.steps,
+            "warmup": args.warmup, "warmup_run": warm_run, "ms_per_step": ms_max / timed, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 state / f64 cell sums + collision" if args.precision == "mixed" else "f64",
             "data": "synthetic", "config": workload_config(args, cfg),
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu,
-            "check": {"kT": kT, "momentum_per_particle": float(np.max(np.abs(P)) / N), "sorts": stats["sorts"], "max_occupancy": stats["max_occupancy"]},
+            "check": {"kT": kT, "momentum_per_particle": float(np.max(np.abs(Pm)) / N), "sorts": stats["sorts"], "sorts_in_timed_region": int(sorts_timed), "sort_period": P, "max_occupancy": stats["max_occupancy"]},
         }
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -33,3 +33,22 @@ def test_reference_arm_other_ranks_exit_quietly_and_configs_are_selectable():
     for cfg, word in (("C4", "MPCD-AT"), ("C5", "chains of 50 beads")):
         d = json.loads(_run("--impl", "reference", "--config", cfg, "--steps", "1", "--warmup", "3", "--ref-particles", "20000")[0])
         assert d["config"]["workload"].startswith(cfg) and word in d["config"]["workload"]
+
+
+def test_all_core_oracle_timing_runs_one_process_per_core():
+    sys.path.insert(0, ROOT)
+    import bench
+    cfg = bench.synth.CONFIGS["C3"]
+    value, cores, n_each = bench.oracle_all_cores(cfg, "mixed", 2, 1, (8, 8, 8))
+    assert cores == len(os.sched_getaffinity(0)) and value > 0 and n_each == 8 * 8 * 8 * cfg["M"]
+
+
+def test_ncu_traffic_is_only_quoted_for_the_kernel_sources_it_was_taken_on():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert len(bench.csrc_hash()) == 16
+    for row in open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")).read().splitlines()[1:]:
+        w = [x.strip() for x in row.split(",")]
+        value, note = bench.ncu_traffic(w[0], w[1], int(w[2]))
+        assert (value is not None) == (w[4] == bench.csrc_hash()), note
+    assert bench.ncu_traffic("C1", "mixed", 0) == (None, "no ncu capture committed for this workload")

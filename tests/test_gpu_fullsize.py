@@ -1,9 +1,10 @@
 """GPU parity and invariants at BASELINE.json's full sizes, in the launch configuration bench.py
 times (mpcd_step: the fused one-pass-per-step pipeline, sort every 25).
 
-C3 / C4 (80 M / 42 M particles): the C oracle still finishes one step in seconds, so the first
-steps are compared ELEMENT BY ELEMENT (positions and cell indices bit-exact, velocities within the
-north_star tolerance), plus the size-independent properties: counts sum to N, momentum conserved.
+C3 / C4 / C5 (80 M / 42 M / 5 M + 50 000 beads): the C oracle still finishes one step in seconds, so the
+first steps are compared ELEMENT BY ELEMENT (positions and cell indices bit-exact, velocities within the
+north_star tolerance; over two steps every mismatch must be explained, tests/parity_explain.py), in both
+precision models, plus the size-independent properties: counts sum to N, momentum conserved.
 C2 (2.6 M particles, 1000 steps): the multi-step invariants of north_star -- total-momentum drift
 <= 1e-6 relative (reading A25) and temperature within statistical error (SRD conserves energy,
 PAPER.md:45)."""
@@ -11,6 +12,7 @@ import numpy as np
 import pytest
 
 import workloads as synth
+from parity_explain import explained_compare
 
 pytestmark = pytest.mark.gpu
 
@@ -44,31 +46,17 @@ def _compare(g, o, tol):
     return err
 
 
-def _compare_multistep(g, o, box, tol):
-    """Several steps from an identical state.  A velocity that differs by one fp32 ulp after the first step
-    (fp64 summation order, allowed by the tolerance) moves the next position by ulp * dt, and at 10^8
-    particles a handful of those land on the other side of a cell boundary, which changes the mean of two
-    cells.  So: positions within 2 ulp of the box length (minimum image), and all but a 1e-5 fraction of
-    cell indices / velocities in agreement."""
+def _compare_multistep(g, o, box, tol, dtype=np.float32):
+    """Two steps from an identical state: every mismatch must be explained by the only legitimate chain (a velocity
+    differing in its last bit -> a position differing by an ulp -> a particle on a cell face binned next door ->
+    another mean for the members of the two cells); see tests/parity_explain.py.  Anything else fails."""
     s = g.get_state()
     a, b = np.argsort(s["tag"], kind="stable"), np.argsort(o.tag, kind="stable")
     assert np.array_equal(s["tag"][a], o.tag[b])
     N = a.size
-    L = np.asarray(box, dtype=np.float64)
-    bad_cell = bad_vel = 0
-    worst_pos = 0.0
-    for lo in range(0, N, 1 << 24):
-        sl = slice(lo, lo + (1 << 24))
-        d = np.abs(s["pos"][a[sl]][:, :3].astype(np.float64) - o.pos[b[sl]][:, :3].astype(np.float64))
-        d = np.minimum(d, L - d)
-        worst_pos = max(worst_pos, float(d.max()))
-        bad_cell += int(np.count_nonzero(s["cell"][a[sl]] != o.cell[b[sl]]))
-        dv = np.abs(s["vel"][a[sl]][:, :3].astype(np.float64) - o.vel[b[sl]][:, :3].astype(np.float64)).max(axis=1)
-        bad_vel += int(np.count_nonzero(dv > tol))
-    assert worst_pos <= 2 * np.spacing(np.float32(L.max())), worst_pos
-    assert bad_cell <= 1e-5 * N, bad_cell
-    assert bad_vel <= 1e-4 * N, bad_vel
-    return bad_cell, bad_vel
+    r = explained_compare(s["pos"][a], s["vel"][a], s["cell"][a], o.pos[b], o.vel[b], o.cell[b], g.get_shift(), 1.0, box, tol, dtype)
+    assert r["bad_cell"] <= 1e-5 * N and r["bad_vel"] <= 40 * max(r["touched_cells"], 1), r
+    return r
 
 
 def test_config3_full_size_first_steps_match_the_oracle(oracle):
@@ -92,9 +80,10 @@ def test_config3_full_size_first_steps_match_the_oracle(oracle):
     assert np.max(np.abs(c["u"] - o.u)) <= 1e-12
     assert np.max(np.abs(c["axis"] - o.axis)) <= 4e-15
     assert g.stats()["max_occupancy"] == int(o.count.max())
-    # a second, fused step (collide(t) + stream + bin(t+1) in one kernel) from the same state
-    st = g.get_state()
-    P0 = st["vel"][:, :3].astype(np.float64).sum(axis=0)
+    del c
+    # two more steps from this common state: the steady-state kernel bench.py times (collide(t) + stream + bin(t+1) in one
+    # launch, particle_pass<float, kSRD|kStream|kBin|kEnergy>), every mismatch explained
+    P0 = g.get_state(pos=False, tag=False, cell=False)["vel"][:, :3].astype(np.float64).sum(axis=0)
     g.step(2); o.step(2)
     _compare_multistep(g, o, [200.0] * 3, 1e-5)
     P1 = g.get_state(pos=False, tag=False, cell=False)["vel"][:, :3].astype(np.float64).sum(axis=0)
@@ -102,12 +91,49 @@ def test_config3_full_size_first_steps_match_the_oracle(oracle):
     g.close()
 
 
+def test_config3_full_size_fused_kernel_teacher_forced(oracle):
+    """The fused steady-state kernel at full size, ELEMENT BY ELEMENT.  With deterministic accumulation (64-bit fixed-point
+    cell sums) a trajectory does not depend on how the steps are split over calls, so mpcd_step(1) x 2 (unfused kernels
+    only) and mpcd_step(2) (the fused kernel in the middle, the sort on its way out: kSortOut) must agree bit for bit; and
+    the oracle, started from the state after the first step, must land on the second: positions and cells bit-exact,
+    velocities within the north_star tolerance."""
+    from paper_1801_10187_b200 import MPCD
+    cfg = synth.CONFIGS["C3"]
+    pos, vel, tag = synth.solvent(cfg["n"], cfg["M"], seed=cfg["seed"], dtype=np.float32)
+    box = [float(x) for x in cfg["n"]]
+    N = pos.shape[0]
+    ga = MPCD(box, N, seed=cfg["seed"], deterministic=True, init_state=False)
+    ga.set_state(pos, vel, tag)
+    ga.step(1)
+    s1 = ga.get_state(cell=False)
+    o = oracle.OracleMPCD(box, N, seed=cfg["seed"], dtype=np.float32, init=False)
+    o.set_state(s1["pos"], s1["vel"], s1["tag"], step=1)
+    del s1
+    ga.step(1)
+    gb = MPCD(box, N, seed=cfg["seed"], deterministic=True, init_state=False)
+    gb.set_state(pos, vel, tag)
+    del pos, vel
+    gb.step(2)
+    sa, sb = ga.get_state(), gb.get_state()
+    ga.close()
+    ia, ib = np.argsort(sa["tag"], kind="stable"), np.argsort(sb["tag"], kind="stable")
+    for k in ("pos", "vel", "cell"):
+        assert np.array_equal(sa[k][ia], sb[k][ib]), f"{k}: mpcd_step(1) x 2 and mpcd_step(2) differ"
+    del sa, sb, ia, ib
+    o.step(1)
+    _compare(gb, o, 1e-5)
+    gb.close()
+
+
 def test_config4_full_size_andersen_thermostat_step(oracle):
     """C4: 256 x 256 x 128 cells, density 5, 42 M particles, AT collision keyed by (seed, step, tag)."""
     g, o, N = _pair(oracle, "C4", np.float32)
     g.step(1); o.step(1)
     _compare(g, o, 1e-5)
-    g.step(2); o.step(2)                 # the fused AT kernel (apply(t) + stream + bin + draw(t+1))
+    st = g.get_state(cell=False)                      # teacher-force, then two steps through the fused AT kernel
+    o.set_state(st["pos"], st["vel"], st["tag"], step=1)
+    del st
+    g.step(2); o.step(2)                 # apply(t) + stream + bin + draw(t+1) in one launch
     _compare_multistep(g, o, [256.0, 256.0, 128.0], 1e-5)
     P, KE, kT = g.get_thermo()
     assert abs(kT - 1.0) < 5e-3          # one AT collision thermalises to kT (statistical error ~ 3e-4 here)
@@ -115,45 +141,61 @@ def test_config4_full_size_andersen_thermostat_step(oracle):
     g.close()
 
 
-def test_config3_fp64_mode_sampled_cells(oracle):
-    """C3 in the all-fp64 model: one fused step, checked on sampled cells the oracle computes one by
-    one (its per-cell definition written out in numpy fp64) and on the global invariants."""
+def test_config3_fp64_model_full_size_through_mpcd_step(oracle):
+    """C3 in the all-fp64 model, element by element against the oracle, through mpcd_step: two steps from t = 0 run
+    particle_pass<double, ...|kSortOut> (the sort of step 0 on the fused kernel's way out), two more the plain fused kernel
+    particle_pass<double, kSRD|kStream|kBin|kEnergy>.  In double a last-bit difference never reaches a cell face, so the
+    comparison is strict: positions 1e-12, cells bit-exact, velocities 1e-12."""
+    g, o, N = _pair(oracle, "C3", np.float64)
+    P0 = o.vel[:, :3].sum(axis=0)
+    K0 = float((o.vel[:, :3] ** 2).sum())
+    for _ in range(2):
+        g.step(2); o.step(2)
+        s = g.get_state()
+        a, b = np.argsort(s["tag"], kind="stable"), np.argsort(o.tag, kind="stable")
+        assert np.array_equal(s["cell"][a], o.cell[b]), "cell indices are not bit-exact"
+        for k, ref in (("pos", o.pos), ("vel", o.vel)):
+            err = 0.0
+            for lo in range(0, N, 1 << 23):
+                sl = slice(lo, lo + (1 << 23))
+                err = max(err, float(np.max(np.abs(s[k][a[sl]][:, :3] - ref[b[sl]][:, :3]))))
+            assert err <= 1e-12, (k, err)
+        P1 = s["vel"][:, :3].sum(axis=0)
+        K1 = float((s["vel"][:, :3] ** 2).sum())
+        del s, a, b
+        assert np.max(np.abs(P1 - P0)) / N <= 1e-15
+        assert abs(K1 - K0) / K0 <= 1e-13          # SRD conserves energy (PAPER.md:45)
+    assert g.stats()["sorts"] == 1 and g.stats()["step"] == 4
+    g.close()
+
+
+def test_config5_full_size_polymer_solution(oracle):
+    """BASELINE config 5 at full size: 100^3 cells, 5 M solvent particles + 1000 chains of 50 beads (mass 5, k = 1000,
+    r0 = 0.5, 10 velocity-Verlet substeps per collision), mixed precision, two steps through mpcd_step (the fused
+    solvent kernel with kEmbedded beside the bead kernel): beads to 1e-11, bead cells bit-exact, solvent within the
+    north_star tolerance with every mismatch explained."""
     from paper_1801_10187_b200 import MPCD
-    cfg = synth.CONFIGS["C3"]
-    pos, vel, tag = synth.solvent(cfg["n"], cfg["M"], seed=cfg["seed"], dtype=np.float64)
-    N = pos.shape[0]
+    cfg = synth.CONFIGS["C5"]
+    ch = cfg["chains"]
+    pos, vel, tag = synth.solvent(cfg["n"], cfg["M"], seed=cfg["seed"], dtype=np.float32)
+    bp, bv, bm = synth.chains(cfg["n"], ch["n_chains"], ch["chain_len"], seed=cfg["seed"] + 1, mass=ch["mass"], r0=ch["r0"])
     box = [float(x) for x in cfg["n"]]
-    g = MPCD(box, N, seed=cfg["seed"], precision="fp64", sort_period=0, init_state=False)
-    g.set_state(pos, vel, tag)
-    g.stream(); g.shift_and_bin()
-    s = g.get_state()
-    shift = g.get_shift()
-    cell_o = oracle.bin_cells(s["pos"], shift, 1.0, cfg["n"])
-    assert np.array_equal(s["cell"], cell_o)
-    c = g.get_cells()
-    assert int(c["count"].sum()) == N
-    rng = np.random.default_rng(1)
-    sample = rng.choice(c["count"].size, size=64, replace=False)
-    members = {int(k): np.flatnonzero(cell_o == k) for k in sample}
-    axis = oracle.draw_axis(cfg["seed"], 0, c["count"].size)
-    g.collide_srd(np.deg2rad(130.0))
-    v1 = g.get_state(pos=False, tag=False, cell=False)["vel"]
-    ca, sa = np.cos(np.deg2rad(130.0)), np.sin(np.deg2rad(130.0))
-    for k, idx in members.items():
-        assert c["count"][k] == idx.size
-        if idx.size == 0:
-            continue
-        v = s["vel"][idx, :3]
-        u = v.sum(axis=0) / idx.size
-        np.testing.assert_allclose(c["u"][k], u, rtol=0, atol=1e-13)
-        n = axis[k]
-        w = v - u
-        wr = w * ca + np.cross(n, w) * sa + np.outer(w @ n, n) * (1.0 - ca)
-        np.testing.assert_allclose(v1[idx, :3], u + wr, rtol=0, atol=1e-12)
-    P0 = s["vel"][:, :3].sum(axis=0); P1 = v1[:, :3].sum(axis=0)
-    assert np.max(np.abs(P1 - P0)) / N <= 1e-15
-    K0 = (s["vel"][:, :3] ** 2).sum(); K1 = (v1[:, :3] ** 2).sum()
-    assert abs(K1 - K0) / K0 <= 1e-13          # SRD conserves energy (PAPER.md:45)
+    N = pos.shape[0]
+    assert N == 5_000_000 and bm.size == 50_000
+    g = MPCD(box, N, seed=cfg["seed"], init_state=False)
+    g.set_state(pos, vel, tag); g.set_embedded(bp, bv, bm, ch["chain_len"], ch["k"], ch["r0"], ch["md_substeps"])
+    o = oracle.OracleMPCD(box, N, seed=cfg["seed"], dtype=np.float32, init=False)
+    o.set_state(pos, vel, tag); o.set_embedded(bp, bv, bm, ch["chain_len"], ch["k"], ch["r0"], ch["md_substeps"])
+    P0 = vel[:, :3].astype(np.float64).sum(axis=0) + (bm[:, None] * bv).sum(axis=0)
+    g.step(2); o.step(2)
+    e = g.get_embedded()
+    assert np.max(np.abs(e["pos"] - o.emb["pos"])) <= 1e-11
+    assert np.max(np.abs(e["vel"] - o.emb["vel"])) <= 1e-11
+    assert np.array_equal(e["cell"], o.emb["cell"])
+    _compare_multistep(g, o, box, 1e-5)
+    s = g.get_state(pos=False, tag=False, cell=False)
+    P1 = s["vel"][:, :3].astype(np.float64).sum(axis=0) + (bm[:, None] * e["vel"]).sum(axis=0)
+    assert np.max(np.abs(P1 - P0)) / (N + ch["mass"] * bm.size) <= 1e-8        # total momentum incl. the beads
     g.close()
 
 

@@ -79,3 +79,53 @@ def test_thermostat_off_has_no_xi():
         g.get_xi()
     assert e.value.code == -4
     g.close()
+
+
+def _vel_err(g, o, strict=True):
+    s = g.get_state()
+    a, b = np.argsort(s["tag"]), np.argsort(o.tag)
+    assert np.array_equal(s["cell"][a], o.cell[b])
+    if strict:                           # one step from a common state: positions bit-exact
+        assert np.array_equal(s["pos"][a][:, :3], o.pos[b][:, :3])
+    return float(np.max(np.abs(s["vel"][a][:, :3].astype(np.float64) - o.vel[b][:, :3].astype(np.float64))))
+
+
+def test_scale_factors_are_redrawn_when_the_same_step_is_binned_again(oracle):
+    """A bin of step s before the step itself (mpcd_get_thermo / mpcd_shift_and_bin on the unstreamed state) computes xi
+    from a membership that mpcd_step then replaces: the step must not reuse those factors.  Likewise a handle reused
+    through mpcd_set_state(step = 0) with another fluid."""
+    g, o = _pair(oracle, (11, 10, 9), 8, 31, np.float32, kT=1.0, kT_init=1.7)
+    g.get_thermo()                       # bins step 0 on the unstreamed state, draws xi(0) from it
+    g.shift_and_bin(); g.get_xi()
+    g.step(1); o.step(1)
+    assert _vel_err(g, o) <= 1e-5 * 2.0
+    pos, vel, tag = synth.solvent((11, 10, 9), 8, seed=77, kT=0.6, dtype=np.float32)      # another fluid, same handle, step 0 again
+    g.set_state(pos, vel, tag, step=0); o.set_state(pos, vel, tag, step=0)
+    g.step(1); o.step(1)
+    assert _vel_err(g, o) <= 1e-5 * 2.0
+    g.set_state(pos, vel, tag, step=0); o.set_state(pos, vel, tag, step=0)                # and once more: same input, same output
+    g.step(2); o.step(2)
+    assert _vel_err(g, o, strict=False) <= 3e-5 * 2.0
+    g.close()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_scale_factors_with_a_drifting_fluid(oracle, dtype):
+    """E_rel = KE - M_c u^2 / 2 in one pass (reading A12) cancels when the fluid drifts; at a drift of 5 sigma the one-pass
+    value still agrees with the oracle's two-pass definition (eq. 3) to 1e-8 relative in the fp64 sums."""
+    n, M = (10, 9, 8), 8
+    pos, vel, tag = synth.solvent(n, M, seed=12, dtype=dtype)
+    vel[:, :3] += np.array([5.0, -3.0, 4.0], dtype=dtype)
+    from paper_1801_10187_b200 import MPCD
+    box = [float(x) for x in n]
+    g = MPCD(box, pos.shape[0], seed=12, precision="fp64" if dtype == np.float64 else "mixed", init_state=False, thermostat=True)
+    o = oracle.OracleMPCD(box, pos.shape[0], seed=12, dtype=dtype, init=False, thermostat=True)
+    g.set_state(pos, vel, tag); o.set_state(pos, vel, tag)
+    g.stream(); o.stream(); g.shift_and_bin(); o.shift_and_bin()
+    np.testing.assert_allclose(g.get_xi(), o.xi, rtol=1e-8)
+    c = g.get_cells()
+    np.testing.assert_allclose(c["kTc"], o.kTc, rtol=1e-8, atol=1e-12)
+    g.collide_srd(math.radians(130.0)); o.collide_srd(math.radians(130.0))
+    tol = 1e-11 if dtype == np.float64 else 1e-5 * 8.0      # |v| ~ 8 sigma: one fp32 ulp is 9.5e-7
+    assert _vel_err(g, o) <= tol * max(1.0, float(np.max(o.xi)))
+    g.close()
