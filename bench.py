@@ -381,7 +381,7 @@ def main():
         t = torch.tensor([wall], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        nbytes = int(sum(x.numel() * x.element_size() for x in bufs[0].values()))
+        nbytes = int(sum(bufs[0][k].numel() * bufs[0][k].element_size() for k in ("pos", "vel", "tag")))
         e2e = {"value": world * N * args.e2e_steps / float(t.item()), "unit": UNIT,
                "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                "steps": args.e2e_steps, "ms_per_step": float(t.item()) / args.e2e_steps * 1e3,
