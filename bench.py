@@ -100,7 +100,8 @@ def ncu_traffic(workload: str, precision: str, brick: int):
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the GPU arm (B200_PROFILING.md recipe), sampled every 10 ms from
     before the warm-up to after the per-kernel timing leg (all of it back-to-back GPU work around the timed region).
-    `sm_mhz` is the median over the samples taken under load (utilization.gpu >= 50 %)."""
+    `sm_mhz` is the median over the samples taken under load (utilization.gpu >= 50 %, which nvidia-smi averages over its own
+    window and so lags, or power.draw >= 250 W)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,utilization.gpu,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -149,9 +150,9 @@ class ClockSampler:
         except Exception:
             pass
         if rows:
-            load = [r for r in rows if r[3] >= 50.0] or rows
+            load = [r for r in rows if r[3] >= 50.0 or r[2] >= 250.0] or rows
             out.update(sm_mhz=float(np.median([r[0] for r in load])), sm_max_mhz=float(max(r[1] for r in rows)), reasons=sorted(reasons),
-                       samples=len(rows), samples_under_load=len([r for r in rows if r[3] >= 50.0]), power_w_max=float(max(r[2] for r in rows)))
+                       samples=len(rows), samples_under_load=len([r for r in rows if r[3] >= 50.0 or r[2] >= 250.0]), power_w_max=float(max(r[2] for r in rows)))
         return out
 
 

@@ -841,19 +841,19 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     const unsigned fb = (emb ? kEmbedded : 0u) | fixed_flag(h);    // flags of the SRD gather; kFixed also goes with every kBin
     const unsigned ft = (!at && thermostatted(h)) ? kThermo : 0u;
     const unsigned fe = (h->opt.cell_energy != 0 || ft) ? kEnergy : 0u;      // the thermostat needs the cell energies
-    int rc = at ? ensure_at_buffers(h) : MPCD_OK;
-    if (rc) return rc;
+    int rc = MPCD_OK;
     uint64_t t = h->step;
     int set = (int)(t & 1);                         // cell arrays of step k: set k & 1
     PassPlan pl;
     pl.alpha = h->opt.alpha;
     // first block: stream + bin + accumulate for step t
-    rc = prepare(h, set, true, at, !at, t);         // zeroed set of step t, axes of step t
+    // (AT: inside this call a cell's ONE accumulator holds sum(v) - sum(dv), kATStored; the second array is not touched)
+    rc = prepare(h, set, true, false, !at, t);      // zeroed set of step t, axes of step t
     if (rc) return rc;
     shift_for(h, t, pl.shift);
     pl.cset = pl.bset = set;
     pl.step_collide = pl.step_bin = t;
-    h->zeroed[set] = false; if (at) h->at_zeroed[set] = false;
+    h->zeroed[set] = false;
     h->xi_valid[set] = false;
     rc = pass(h, kStream | kBin | fe | fixed_flag(h) | (at ? (kATDraw | kATStored) : 0u), pl);   // AT: vel.xyz carries dv between the launches of this call
     if (!rc && emb) rc = emb_step_launch<kEmbMd | kEmbBinAcc>(h, set, set, t, pl.shift, h->opt.alpha);
@@ -864,7 +864,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     // stream + bin + accumulate (t + 1)
     for (int32_t j = 1; j < nsteps; ++j) {
         const int nxt = set ^ 1;
-        rc = prepare(h, nxt, true, at, !at, t + 1);
+        rc = prepare(h, nxt, true, false, !at, t + 1);
         if (rc) return rc;
         if (sort_pending) { rc = scan_counts(h, set); if (rc) return rc; }
         shift_for(h, t + 1, pl.shift);
@@ -874,7 +874,7 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
         }
         pl.cset = set; pl.bset = nxt;
         pl.step_collide = t; pl.step_bin = t + 1;
-        h->zeroed[nxt] = false; if (at) h->at_zeroed[nxt] = false;
+        h->zeroed[nxt] = false;
         h->xi_valid[nxt] = false;
         rc = pass(h, (at ? (kATApply | kATDraw | kATStored) : (kSRD | ft | fb)) | kStream | kBin | fe | (sort_pending ? kSortOut : 0u), pl);
         if (rc) return rc;

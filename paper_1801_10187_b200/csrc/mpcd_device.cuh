@@ -305,19 +305,24 @@ template <> struct AccOps<long long> {
 
 // kExtra: a second triple (ex, ey, ez), already double, is summed over the same groups into xacc[c] = {X, Y, Z, -} by the
 // same match and the same tree (the AT rule's sum of the thermostat draws), instead of a second pass.
-template <typename T, bool kCount, bool kEnergy, bool kFixed = false, bool kExtra = false>
+// kMinus: a second NATIVE triple (gx, gy, gz) is subtracted from the first before the summation (the difference of two
+// native values is formed in double: exact), while the energy stays that of the first triple: inside mpcd_step the AT rule
+// needs only sum(v) - sum(dv) of a cell (eq. 4: v' = (S - D) / N_c + dv), so ONE sum per cell carries both.
+template <typename T, bool kCount, bool kEnergy, bool kFixed = false, bool kExtra = false, bool kMinus = false>
 __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, double *__restrict__ qacc,
                                                      typename std::conditional<kExtra, WarpScratchX, WarpScratch>::type &ws,
                                                      int c /* < 0 = inactive lane, unique per lane */, T fx, T fy, T fz,
-                                                     double *__restrict__ xacc = nullptr, double ex = 0.0, double ey = 0.0, double ez = 0.0)
+                                                     double *__restrict__ xacc = nullptr, double ex = 0.0, double ey = 0.0, double ez = 0.0,
+                                                     T gx = T(0), T gy = T(0), T gz = T(0))
 {
     static_assert(!(kExtra && kFixed), "the second triple is summed in double");
+    static_assert(!(kMinus && (kExtra || kFixed)), "the difference is summed in double, alone");
     using A = typename std::conditional<kFixed, long long, double>::type;
     using Ops = AccOps<A>;
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const double dx0 = (double)fx, dy0 = (double)fy, dz0 = (double)fz;
-    A vx = Ops::from(dx0), vy = Ops::from(dy0), vz = Ops::from(dz0);
+    A vx = Ops::from(kMinus ? dx0 - (double)gx : dx0), vy = Ops::from(kMinus ? dy0 - (double)gy : dy0), vz = Ops::from(kMinus ? dz0 - (double)gz : dz0);
     A q = kEnergy ? Ops::from(sq_norm(dx0, dy0, dz0)) : A(0);
     unsigned peers = __match_any_sync(full, c);
     const int size = __popc(peers);
@@ -329,12 +334,13 @@ __device__ __forceinline__ void warp_cell_accumulate(double *__restrict__ acc, d
         const int next = __ffs(peers);                     // 1-based lane of the next peer, 0 = none
         const int src = next ? next - 1 : lane;
         const T tx = __shfl_sync(full, fx, src), ty = __shfl_sync(full, fy, src), tz = __shfl_sync(full, fz, src);
+        const T sx = kMinus ? __shfl_sync(full, gx, src) : T(0), sy = kMinus ? __shfl_sync(full, gy, src) : T(0), sz = kMinus ? __shfl_sync(full, gz, src) : T(0);
         alive = !(rank & 1);
         const double ux = kExtra ? __shfl_sync(full, ex, src) : 0.0, uy = kExtra ? __shfl_sync(full, ey, src) : 0.0,
                      uz = kExtra ? __shfl_sync(full, ez, src) : 0.0;
         if (next && alive) {
             const double dx = (double)tx, dy = (double)ty, dz = (double)tz;
-            vx += Ops::from(dx); vy += Ops::from(dy); vz += Ops::from(dz);
+            vx += Ops::from(kMinus ? dx - (double)sx : dx); vy += Ops::from(kMinus ? dy - (double)sy : dy); vz += Ops::from(kMinus ? dz - (double)sz : dz);
             if (kEnergy) q += Ops::from(sq_norm(dx, dy, dz));
             if (kExtra) { ex += ux; ey += uy; ez += uz; }
         }

@@ -14,7 +14,9 @@
 //                    Alg. 1 lines 8-10 PAPER.md:150-152); xi rides in the 4th word of the cell's axis sector
 //   kATStored a7     inside mpcd_step: kATDraw leaves the drawn dv in vel.xyz instead of the velocity (the AT update
 //                    v = u + dv - D/N_c does not depend on the old velocity, which has been summed by then), and the
-//                    next kATApply takes it from there instead of regenerating it: one Gaussian draw per particle-step
+//                    next kATApply takes it from there instead of regenerating it: one Gaussian draw per particle-step;
+//                    the cell's accumulator then holds sum(v) - sum(dv) (all that eq. 4 needs: v' = (S - D) / N_c + dv),
+//                    so there is one sum, one combining tree and one gathered sector per particle instead of two
 //   kEmbedded a5     with kSRD: the cell mean is mass-weighted over the solvent sums and the embedded beads' sums
 //                    (mpcd_embedded.cuh)
 //   kFixed    a4     deterministic accumulation: the cell sums are 64-bit fixed-point integers (mpcd_device.cuh), both
@@ -99,7 +101,7 @@ template <typename T, unsigned F>
 __global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_F32 : MPCD_MINBLOCKS_F64) particle_pass(const PassArgs<T> a)
 {
     using V4 = typename Vec4<T>::type;
-    using WS = typename std::conditional<(F & kBin) && (F & kATDraw), WarpScratchX, WarpScratch>::type;
+    using WS = typename std::conditional<(F & kBin) && (F & kATDraw) && !(F & kATStored), WarpScratchX, WarpScratch>::type;
     __shared__ WS ws[(F & (kBin | kATDraw)) ? kPassThreads / 32 : 1];
     WS &w = ws[(F & (kBin | kATDraw)) ? (threadIdx.x >> 5) : 0];
     const int64_t i = (int64_t)blockIdx.x * kPassThreads + threadIdx.x;
@@ -136,19 +138,19 @@ __global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_
     if (F & kATApply) {
         {                                                        // eq. 4: v = u + dv_i - D / N_c = (S - D) / N_c + dv_i
             const f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);
-            const f64x4 d = ld256_nc(a.dsum + 4 * (size_t)c);
             const double inv = __drcp_rn(s.w);
-            double dx, dy, dz;                                   // dv_i of the step being collided
-            if (F & kATStored) {
-                dx = (double)v.x; dy = (double)v.y; dz = (double)v.z;
+            if (F & kATStored) {                                 // inside mpcd_step the cell's one sum IS S - D (kMinus below), dv_i rides in vel.xyz
+                v.x = (T)(s.x * inv + (double)v.x);
+                v.y = (T)(s.y * inv + (double)v.y);
+                v.z = (T)(s.z * inv + (double)v.z);
             } else {
-                double g0, g1, g2;
+                const f64x4 d = ld256_nc(a.dsum + 4 * (size_t)c);
+                double g0, g1, g2;                               // dv_i of the step being collided
                 draw_gauss3<T>(a.seed, a.step_collide, tag, g0, g1, g2);
-                dx = a.sigma * g0; dy = a.sigma * g1; dz = a.sigma * g2;
+                v.x = (T)((s.x - d.x) * inv + a.sigma * g0);
+                v.y = (T)((s.y - d.y) * inv + a.sigma * g1);
+                v.z = (T)((s.z - d.z) * inv + a.sigma * g2);
             }
-            v.x = (T)((s.x - d.x) * inv + dx);
-            v.y = (T)((s.y - d.y) * inv + dy);
-            v.z = (T)((s.z - d.z) * inv + dz);
         }
     }
     if (F & kStream) {
@@ -177,7 +179,9 @@ __global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_
     if ((F & (kSRD | kATApply | kBin)) && valid) store4(((F & kSortOut) ? a.vel_out : a.vel) + o, vs);
     if ((F & kSortOut) && valid) a.tag_out[o] = tag;
     if (!valid) c = inactive;                                    // takes no part in the sums
-    if constexpr ((F & kBin) && (F & kATDraw))          // one match and one tree for both sums: same cell, same groups
+    if constexpr ((F & kBin) && (F & kATDraw) && (F & kATStored))   // ONE sum per cell: sum(v) - sum(dv) is all eq. 4 needs; the stored dv is what is subtracted
+        warp_cell_accumulate<T, true, (F & kEnergy) != 0, false, false, true>(a.acc, a.qacc, w, c, v.x, v.y, v.z, nullptr, 0.0, 0.0, 0.0, vs.x, vs.y, vs.z);
+    else if constexpr ((F & kBin) && (F & kATDraw))     // one match and one tree for both sums: same cell, same groups
         warp_cell_accumulate<T, true, (F & kEnergy) != 0, false, true>(a.acc, a.qacc, w, c, v.x, v.y, v.z, a.at_acc, ex, ey, ez);
     else if constexpr ((F & kBin) != 0) warp_cell_accumulate<T, true, (F & kEnergy) != 0, (F & kFixed) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
     else if constexpr ((F & kATDraw) != 0) warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, ex, ey, ez);
