@@ -188,8 +188,10 @@ int mpcd_get_shift(mpcd_t *h, double s[3]);
  * their cell's axis like the solvent -- and wherever the solvent streams over dt (mpcd_stream, mpcd_step) the beads
  * are advanced by md_substeps velocity-Verlet steps of dt / md_substeps.  Beads are kept in double whatever the
  * precision model (A27).  pos3, vel3: HOST, nb x 3 doubles, positions in [0, box); mass: HOST, nb doubles.  Needs the
- * SRD rule without the cell thermostat (MPCD_EINVAL otherwise); the sort leaves the beads alone;
- * mpcd_get_cells / mpcd_get_thermo report the solvent only.  Calling it again with the same nb replaces the state. */
+ * SRD rule without deterministic accumulation (MPCD_EINVAL otherwise); the sort leaves the beads alone;
+ * mpcd_get_cells / mpcd_get_thermo report the solvent only.  With opt.thermostat = 1 the beads are particles of their cell
+ * for the thermostat too (A28): E_k of eq. 3 sums m_i |v_i - u|^2 / 2 over solvent and beads,
+ * the drawn energy follows the cell's particle count incl. beads, and xi scales the beads' relative velocities as well.  Calling it again with the same nb replaces the state. */
 int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *vel3, const double *mass, int32_t chain_len, double k, double r0,
                       int32_t md_substeps);
 /* Bead state to HOST buffers (any may be NULL): pos3, vel3 nb x 3 doubles, cell nb x i32 (last binning).  Synchronises. */

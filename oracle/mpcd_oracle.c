@@ -37,7 +37,10 @@
  * pinned Philox words, KS tests, zero net momentum; the rotation sense inside
  * oracle_collide_srd_beads against scipy's Rotation; oracle_collide_srd_xi bit-identical to
  * oracle_collide_srd at xi = 1 and doubling the relative velocity at xi = 2
- * (test_oracle_pins_r2.py).
+ * (test_oracle_pins_r2.py); thermostat with beads (oracle_erel_about, oracle_embedded_energy,
+ * oracle_collide_srd_beads_xi): E_k' = E^ per cell incl. the beads, cell momentum kept, agreement with the
+ * pinned plain functions at xi = 1 / without beads, equipartition of hot beads under the thermostat
+ * (test_oracle_embedded.py).
  * parity unpinned: none.
  */
 #include <math.h>
@@ -298,6 +301,44 @@ void oracle_collide_srd_beads(int64_t nb, double *vel3, const int32_t *cell_b, c
         vel3[3 * i + 0] = ux + wx * cos_a + cx * sin_a + nx * ndw * (1.0 - cos_a);
         vel3[3 * i + 1] = uy + wy * cos_a + cy * sin_a + ny * ndw * (1.0 - cos_a);
         vel3[3 * i + 2] = uz + wz * cos_a + cz * sin_a + nz * ndw * (1.0 - cos_a);
+    }
+}
+
+/* ... with the cell thermostat (PAPER.md:157 + :159 "including the solute particles in all stages of the algorithm";
+ * reading A28): the beads' rotated relative velocities are scaled by the cell's xi like the solvent's (Alg. 1 lines 8-10). */
+void oracle_collide_srd_beads_xi(int64_t nb, double *vel3, const int32_t *cell_b, const double *u3, const double *axis3,
+                                 const double *xi, double cos_a, double sin_a)
+{
+    for (int64_t i = 0; i < nb; ++i) {
+        const int64_t c = cell_b[i];
+        const double ux = u3[3 * c], uy = u3[3 * c + 1], uz = u3[3 * c + 2];
+        const double nx = axis3[3 * c], ny = axis3[3 * c + 1], nz = axis3[3 * c + 2];
+        const double wx = vel3[3 * i] - ux, wy = vel3[3 * i + 1] - uy, wz = vel3[3 * i + 2] - uz;
+        const double ndw = nx * wx + ny * wy + nz * wz;
+        const double cx = ny * wz - nz * wy, cy = nz * wx - nx * wz, cz = nx * wy - ny * wx;
+        double rx = wx * cos_a + cx * sin_a + nx * ndw * (1.0 - cos_a);
+        double ry = wy * cos_a + cy * sin_a + ny * ndw * (1.0 - cos_a);
+        double rz = wz * cos_a + cz * sin_a + nz * ndw * (1.0 - cos_a);
+        rx = rx * xi[c]; ry = ry * xi[c]; rz = rz * xi[c];
+        vel3[3 * i + 0] = ux + rx;
+        vel3[3 * i + 1] = uy + ry;
+        vel3[3 * i + 2] = uz + rz;
+    }
+}
+
+/* The beads' share of a cell's relative kinetic energy and member count (eq. 3 PAPER.md:47 with the sum taken over ALL
+ * particles of the cell, solvent and solute; reading A28): erel[c] += sum_beads m_b |v_b - u|^2 / 2 with the
+ * mass-weighted mean u of oracle_embedded_means, ntot[c] = count[c] + beads in c.  erel comes in holding the solvent's share
+ * about the SAME u (oracle_erel_about). */
+void oracle_embedded_energy(int64_t Nc, const int32_t *count, int64_t nb, const int32_t *cell_b, const double *vel3_b, const double *mass_b,
+                            const double *u3, double *erel, int32_t *ntot)
+{
+    for (int64_t c = 0; c < Nc; ++c) ntot[c] = count[c];
+    for (int64_t i = 0; i < nb; ++i) {
+        const int64_t c = cell_b[i];
+        const double wx = vel3_b[3 * i] - u3[3 * c], wy = vel3_b[3 * i + 1] - u3[3 * c + 1], wz = vel3_b[3 * i + 2] - u3[3 * c + 2];
+        erel[c] += 0.5 * mass_b[i] * (wx * wx + wy * wy + wz * wz);
+        ntot[c] += 1;
     }
 }
 

@@ -174,6 +174,21 @@ def collide_srd_beads(vel3, cell_b, u, axis, alpha):
                                    C.c_double(math.sin(alpha)))
 
 
+def collide_srd_beads_xi(vel3, cell_b, u, axis, xi, alpha):
+    lib().oracle_collide_srd_beads_xi(C.c_int64(vel3.shape[0]), _p(vel3), _p(cell_b), _p(u), _p(axis), _p(np.ascontiguousarray(xi, dtype=np.float64)),
+                                      C.c_double(math.cos(alpha)), C.c_double(math.sin(alpha)))
+
+
+def erel_with_beads(vel4, cell, m, count, u, cell_b, vel3_b, mass_b):
+    """NEXT-1 + NEXT-2 (reading A28): relative kinetic energy of every cell over solvent AND beads about the mass-weighted
+    mean u, and the number of particles of the cell (solvent + beads)."""
+    Nc = count.shape[0]
+    erel, ntot = np.empty(Nc), np.empty(Nc, dtype=np.int32)
+    getattr(lib(), "oracle_erel_about" + _suf(vel4.dtype))(C.c_int64(vel4.shape[0]), _p(vel4), _p(cell), C.c_int64(Nc), C.c_double(m), _p(u), _p(erel))
+    lib().oracle_embedded_energy(C.c_int64(Nc), _p(count), C.c_int64(cell_b.shape[0]), _p(cell_b), _p(vel3_b), _p(mass_b), _p(u), _p(erel), _p(ntot))
+    return erel, ntot
+
+
 def collide_at(vel4, cell, Nc, count, u, dv):
     """a7: eq. (4), in place on vel4."""
     getattr(lib(), "oracle_collide_at" + _suf(vel4.dtype))(C.c_int64(vel4.shape[0]), _p(vel4), _p(cell), C.c_int64(Nc), _p(count), _p(u), _p(dv))
@@ -249,7 +264,7 @@ class OracleMPCD:
     def set_embedded(self, pos3, vel3, mass, chain_len, k, r0, md_substeps):
         """NEXT-1 (BASELINE config 5): beads of linear harmonic chains that join the SRD collision and
         move by md_substeps velocity-Verlet steps per collision step.  Beads are kept in double (A27)."""
-        assert self.rule == self.SRD and not self.thermostat
+        assert self.rule == self.SRD
         self.emb = dict(pos=np.ascontiguousarray(pos3, dtype=np.float64).copy(), vel=np.ascontiguousarray(vel3, dtype=np.float64).copy(),
                         mass=np.ascontiguousarray(mass, dtype=np.float64).copy(), chain_len=int(chain_len), k=float(k), r0=float(r0),
                         nsub=int(md_substeps), cell=None)
@@ -282,7 +297,11 @@ class OracleMPCD:
             self._bin_embedded()
             self.u, self.Mc = embedded_means(self.m, self.count, self.sumv, self.emb["cell"], self.emb["vel"], self.emb["mass"])
         if self.thermostat:      # "we compute xi for each cell at the same time that we draw the rotation vectors"
-            self.ehat, self.xi = thermostat_xi(self.seed, self.step_count, self.kT, self.count, self.erel)
+            if self.emb is not None:         # the cell's particles are solvent AND beads (reading A28)
+                self.erel_tot, self.ntot = erel_with_beads(self.vel, self.cell, self.m, self.count, self.u, self.emb["cell"], self.emb["vel"], self.emb["mass"])
+                self.ehat, self.xi = thermostat_xi(self.seed, self.step_count, self.kT, self.ntot, self.erel_tot)
+            else:
+                self.ehat, self.xi = thermostat_xi(self.seed, self.step_count, self.kT, self.count, self.erel)
 
     def sort(self):
         perm = sort_perm(self.cell, self.Nc)
@@ -292,7 +311,10 @@ class OracleMPCD:
     def collide_srd(self, alpha=None):
         alpha = self.alpha if alpha is None else alpha
         if self.emb is not None:
-            collide_srd_beads(self.emb["vel"], self.emb["cell"], self.u, self.axis, alpha)
+            if self.thermostat:
+                collide_srd_beads_xi(self.emb["vel"], self.emb["cell"], self.u, self.axis, self.xi, alpha)
+            else:
+                collide_srd_beads(self.emb["vel"], self.emb["cell"], self.u, self.axis, alpha)
         if self.thermostat:
             collide_srd_xi(self.vel, self.cell, self.u, self.axis, self.xi, alpha)
         else:

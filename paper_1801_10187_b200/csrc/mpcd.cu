@@ -49,6 +49,7 @@ struct mpcd {
     double emb_k = 0, emb_r0 = 0;
     double4 *emb_pos = nullptr, *emb_vel = nullptr;
     double *emb_acc[2] = {nullptr, nullptr};
+    double *emb_q[2] = {nullptr, nullptr};     // {sum m |v|^2, number of beads} per cell: only with the cell thermostat (A28)
     bool emb_zeroed[2] = {false, false};
     bool emb_binned = false;       // the beads are binned and summed for the current bin
     cudaStream_t emb_stream = nullptr;   // inside mpcd_step the bead kernel runs beside the solvent's step kernel (fork / join by events)
@@ -268,6 +269,9 @@ template <typename T> int launch_pass(mpcd_t *h, unsigned F, const PassPlan &pl)
         CASE(kSRD | kEmbedded | kStream | kBin | kEnergy)
         CASE(kSRD | kEmbedded | kStream | kBin | kSortOut)
         CASE(kSRD | kEmbedded | kStream | kBin | kEnergy | kSortOut)
+        CASE(kSRD | kThermo | kEmbedded)
+        CASE(kSRD | kThermo | kEmbedded | kStream | kBin | kEnergy)
+        CASE(kSRD | kThermo | kEmbedded | kStream | kBin | kEnergy | kSortOut)
         CASE(kBin | kEnergy | kFixed)
         CASE(kStream | kBin | kFixed)
         CASE(kStream | kBin | kEnergy | kFixed)
@@ -357,6 +361,8 @@ template <typename T> int launch_brick(mpcd_t *h, unsigned F, const PassPlan &pl
         CASE(kSRD | kEmbedded | kStream | kBin | kEnergy | kSortOut)
         CASE(kSRD | kThermo | kStream | kBin | kEnergy)
         CASE(kSRD | kThermo | kStream | kBin | kEnergy | kSortOut)
+        CASE(kSRD | kThermo | kEmbedded | kStream | kBin | kEnergy)
+        CASE(kSRD | kThermo | kEmbedded | kStream | kBin | kEnergy | kSortOut)
         CASE_F32(kSRD | kStream | kBin | kFixed)
         CASE_F32(kSRD | kStream | kBin | kEnergy | kFixed)
         CASE_F32(kSRD | kStream | kBin | kSortOut | kFixed)
@@ -406,7 +412,7 @@ int prepare(mpcd_t *h, int zset, bool sums, bool at, bool want_axes, uint64_t ax
     ProfScope prof(h, MPCD_PROF_CELLS);
     cell_prepare<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(ax ? h->axis[b] : nullptr, h->seed, axis_step, zs ? h->acc[zset] : nullptr,
                                                            zs ? h->qacc[zset] : nullptr, za ? h->at_acc[zset] : nullptr,
-                                                           ze ? h->emb_acc[zset] : nullptr, h->Nc);
+                                                           ze ? h->emb_acc[zset] : nullptr, ze ? h->emb_q[zset] : nullptr, h->Nc);
     LAUNCH_CHECK(h);
     if (zs) h->zeroed[zset] = true;
     if (za) h->at_zeroed[zset] = true;
@@ -427,7 +433,8 @@ int thermostat(mpcd_t *h, uint64_t t)
     int rc = ensure_axes(h, t);
     if (rc) return rc;
     ProfScope prof(h, MPCD_PROF_CELLS);
-    cell_thermostat<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[b], h->qacc[b], h->axis[b], h->Nc, h->m, h->kT, h->seed, t, deterministic(h));
+    cell_thermostat<<<grid_for(h->Nc, 256), 256, 0, h->stream>>>(h->acc[b], h->qacc[b], h->axis[b], h->Nc, h->m, h->kT, h->seed, t, deterministic(h),
+                                                                 h->emb_acc[b], h->emb_q[b]);
     LAUNCH_CHECK(h);
     h->xi_valid[b] = true;
     return MPCD_OK;
@@ -442,6 +449,8 @@ EmbArgs emb_args(mpcd_t *h, int cset, int bset, uint64_t step_collide, const dou
     e.pos = h->emb_pos; e.vel = h->emb_vel; e.nb = h->emb_n;
     e.sums = h->acc[cset]; e.esum = h->emb_acc[cset]; e.axis = h->axis[step_collide & 1];
     e.eacc = h->emb_acc[bset];
+    e.eqacc = h->emb_q[bset];
+    e.thermo = h->opt.thermostat != 0;
     for (int d = 0; d < 3; ++d) { e.n[d] = h->n[d]; e.shift[d] = shift[d]; }
     e.inv_a = 1.0 / h->a;
     e.mass_solvent = h->m;
@@ -576,8 +585,8 @@ int bin_accumulate(mpcd_t *h, uint64_t t)
     h->ccur = set;
     h->bin_valid = true; h->bin_step = t;
     rc = ensure_axes(h, t);
-    if (!rc && thermostatted(h)) rc = thermostat(h, t);
     if (!rc && embedded(h)) { rc = emb_bin(h, set, pl.shift); h->emb_binned = rc == MPCD_OK; }
+    if (!rc && thermostatted(h)) rc = thermostat(h, t);       // after the beads: they count in the cell's energy (A28)
     if (rc) return rc;
     h->sums_valid = true; h->energy_valid = true; h->counts_valid = true;
     return MPCD_OK;
@@ -975,8 +984,8 @@ int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *v
                       int32_t md_substeps)
 {
     if (!h) return MPCD_EINVAL;
-    if (h->opt.rule != MPCD_SRD || thermostatted(h) || deterministic(h))
-        return fail(h, MPCD_EINVAL, "embedded beads need the SRD rule without the cell thermostat and without deterministic accumulation%s");
+    if (h->opt.rule != MPCD_SRD || deterministic(h))
+        return fail(h, MPCD_EINVAL, "embedded beads need the SRD rule without deterministic accumulation%s");
     if (nb < 1 || !pos3 || !vel3 || !mass || chain_len < 1 || chain_len > kMaxChainLen || nb % chain_len != 0 || !(k >= 0) || !(r0 >= 0) || md_substeps < 1)
         return fail(h, MPCD_EINVAL, "set_embedded: nb >= 1 a multiple of chain_len in [1, 512], k, r0 >= 0, md_substeps >= 1%s");
     std::vector<double4> hp, hv;
@@ -993,6 +1002,7 @@ int mpcd_set_embedded(mpcd_t *h, int64_t nb, const double *pos3, const double *v
         int rc = dev_alloc_t(h, &h->emb_pos, (size_t)nb);
         if (!rc) rc = dev_alloc_t(h, &h->emb_vel, (size_t)nb);
         for (int s = 0; s < 2 && !rc; ++s) { rc = dev_alloc_t(h, &h->emb_acc[s], (size_t)h->Nc * 4); h->emb_zeroed[s] = false; }
+        for (int s = 0; s < 2 && !rc && thermostatted(h); ++s) rc = dev_alloc_t(h, &h->emb_q[s], (size_t)h->Nc * 2);
         if (rc) return rc;
         if (cudaStreamCreateWithFlags(&h->emb_stream, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&h->emb_fork, cudaEventDisableTiming) != cudaSuccess ||

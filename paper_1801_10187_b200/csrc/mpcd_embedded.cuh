@@ -6,6 +6,8 @@
 // pass only learns to add the beads' momentum and mass to its cell mean (flag kEmbedded in mpcd_kernels.cuh).
 //   pos[i] = {x, y, z, mass}        vel[i] = {vx, vy, vz, cell of the last binning (as bits)}
 //   esum[c] = {sum m v (3), sum m} over the beads of cell c: one 32-byte sector, by step parity like the solvent sums
+//   eq[c]   = {sum m |v|^2, number of beads} of cell c (only with the cell thermostat, reading A28: the cell's kinetic
+//             energy and its number of particles count the beads)
 #pragma once
 #include "mpcd_device.cuh"
 
@@ -47,6 +49,8 @@ struct EmbArgs {
     int64_t nb;
     const double *sums, *esum, *axis;    // cell arrays of the step being collided
     double *eacc;                        // bead accumulators of the step being binned
+    double *eqacc;                       // ... {sum m |v|^2, count} (thermostat only, else NULL)
+    int32_t thermo;                      // the rotation scales the relative velocity by the cell's xi (4th word of the axis sector)
     int32_t n[3];
     double shift[3], inv_a, mass_solvent, cos_a, sin_a;
 };
@@ -86,7 +90,7 @@ __global__ void __launch_bounds__(kEmbThreads) emb_step(const MdArgs a, const Em
             const f64x4 s = ld256(e.sums + 4 * c), b = ld256(e.esum + 4 * c), ax = ld256(e.axis + 4 * c);
             double ux, uy, uz;
             embedded_mean(s, b, e.mass_solvent, ux, uy, uz);
-            srd_rotate(v.x, v.y, v.z, ux, uy, uz, ax.x, ax.y, ax.z, 1.0, e.cos_a, e.sin_a, v.x, v.y, v.z);
+            srd_rotate(v.x, v.y, v.z, ux, uy, uz, ax.x, ax.y, ax.z, e.thermo ? ax.w : 1.0, e.cos_a, e.sin_a, v.x, v.y, v.z);
         }
         sx[3 * j] = p.x; sx[3 * j + 1] = p.y; sx[3 * j + 2] = p.z; smass[j] = p.w;
         sv[3 * j] = v.x; sv[3 * j + 1] = v.y; sv[3 * j + 2] = v.z;
@@ -136,6 +140,7 @@ __global__ void __launch_bounds__(kEmbThreads) emb_step(const MdArgs a, const Em
             v.w = __longlong_as_double((long long)c);
             double *q = e.eacc + 4 * (size_t)c;
             atomicAdd(q, p.w * v.x); atomicAdd(q + 1, p.w * v.y); atomicAdd(q + 2, p.w * v.z); atomicAdd(q + 3, p.w);
+            if (e.eqacc) { atomicAdd(e.eqacc + 2 * (size_t)c, p.w * sq_norm(v.x, v.y, v.z)); atomicAdd(e.eqacc + 2 * (size_t)c + 1, 1.0); }
         }
         if (G & kEmbMd) st_d4(a.pos + base + j, p);
         st_d4(a.vel + base + j, v);

@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(256) cells_of_particles(const PassArgs<T> a, i
 // together with the zeroing of the set of step t + 2.
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) cell_prepare(double *axis, uint64_t seed, uint64_t step, double *zero_acc, double *zero_q, double *zero_at, double *zero_emb,
-                                                    int64_t Nc)
+                                                    double *zero_embq, int64_t Nc)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
@@ -211,6 +211,7 @@ __global__ void __launch_bounds__(256) cell_prepare(double *axis, uint64_t seed,
     if (zero_q) zero_q[c] = 0.0;
     if (zero_at) st256(zero_at + 4 * c, 0.0, 0.0, 0.0, 0.0);
     if (zero_emb) st256(zero_emb + 4 * c, 0.0, 0.0, 0.0, 0.0);
+    if (zero_embq) { zero_embq[2 * c] = 0.0; zero_embq[2 * c + 1] = 0.0; }
     if (axis) {
         double nx, ny, nz;
         draw_axis(seed, step, (uint32_t)c, nx, ny, nz);
@@ -223,21 +224,28 @@ __global__ void __launch_bounds__(256) cell_prepare(double *axis, uint64_t seed,
 // from the canonical distribution; xi = 1 for N_c < 2 and for E_k = 0.  Written into the 4th word of the cell's
 // axis sector, which the collision gathers anyway.
 __global__ void __launch_bounds__(256) cell_thermostat(const double *acc, const double *qacc, double *axis, int64_t Nc, double m, double kT,
-                                                       uint64_t seed, uint64_t step, bool fixed)
+                                                       uint64_t seed, uint64_t step, bool fixed, const double *esum, const double *eq)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= Nc) return;
     f64x4 s = ld256(acc + 4 * c);
     s.x = acc_value(s.x, fixed); s.y = acc_value(s.y, fixed); s.z = acc_value(s.z, fixed); s.w = acc_count(s.w, fixed);
-    const int n = (int)s.w;
+    int n = (int)s.w;
+    // kinetic energy, momentum and mass of the cell's particles: the solvent's, plus the embedded beads' (reading A28)
+    double q2 = m * acc_value(qacc[c], fixed), Px = m * s.x, Py = m * s.y, Pz = m * s.z, M = m * s.w;
+    if (esum) {
+        const f64x4 e = ld256(esum + 4 * c);
+        Px += e.x; Py += e.y; Pz += e.z; M += e.w;
+        q2 += eq[2 * c];
+        n += (int)eq[2 * c + 1];
+    }
     double xi = 1.0;
     if (n >= 2) {
         // E_rel = KE - M_c u^2 / 2 (A12) cancels when the cell drifts much faster than it is warm: below 1e-9 of the cell's
         // kinetic energy the difference is rounding noise of the fp64 sums, and the cell is left alone like E_k = 0 (A26)
-        const double q = acc_value(qacc[c], fixed);
-        const double erel = 0.5 * m * (q - (s.x * s.x + s.y * s.y + s.z * s.z) / s.w);
+        const double erel = 0.5 * (q2 - (Px * Px + Py * Py + Pz * Pz) / M);
         const double ehat = draw_cell_energy(seed, step, (uint32_t)c, n, kT);
-        if (erel > 1e-9 * 0.5 * m * q) xi = sqrt(ehat / erel);
+        if (erel > 1e-9 * 0.5 * q2) xi = sqrt(ehat / erel);
     }
     axis[4 * c + 3] = xi;
 }

@@ -101,10 +101,69 @@ def test_config5_like_run_conserves_momentum_and_equilibrates():
     g.close()
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_cell_thermostat_with_beads_matches_the_oracle(oracle, dtype):
+    """Reading A28: the beads count in the cell's kinetic energy and particle number, xi scales their
+    relative velocities too.  Unfused calls: xi to 1e-9 (one-pass E_k against the oracle's two passes), velocities within
+    tolerance; then fused steps through mpcd_step, including the sort on the fused kernel's way out."""
+    n = (9, 8, 7)
+    pos, vel, tag = synth.solvent(n, 5, seed=70, kT=1.5, dtype=dtype)
+    bp, bv, bm = synth.chains(n, 14, 12, seed=71, kT=3.0, mass=MB, r0=R0)
+    box = [float(x) for x in n]
+    from paper_1801_10187_b200 import MPCD
+    kw = dict(sort_period=2)
+    g = MPCD(box, pos.shape[0], seed=70, precision="fp64" if dtype == np.float64 else "mixed", init_state=False, thermostat=True, **kw)
+    g.set_state(pos, vel, tag); g.set_embedded(bp, bv, bm, 12, K, R0, NSUB)
+    o = oracle.OracleMPCD(box, pos.shape[0], seed=70, dtype=dtype, init=False, thermostat=True, **kw)
+    o.set_state(pos, vel, tag); o.set_embedded(bp, bv, bm, 12, K, R0, NSUB)
+    g.stream(); o.stream(); g.shift_and_bin(); o.shift_and_bin()
+    xi = g.get_xi()
+    assert np.all(xi[o.ntot < 2] == 1.0) and np.any((o.count < 2) & (o.ntot >= 2))     # a lone solvent particle with a bead IS thermostatted
+    np.testing.assert_allclose(xi, o.xi, rtol=1e-9)
+    g.collide_srd(math.radians(130.0)); o.collide_srd(math.radians(130.0))
+    tol = (1e-11 if dtype == np.float64 else 1e-5) * max(1.0, float(np.max(o.xi)))
+    np.testing.assert_allclose(g.get_embedded()["vel"], o.emb["vel"], rtol=0, atol=max(tol, 1e-11) if dtype == np.float64 else tol)
+    assert np.max(np.abs(g.get_state()["vel"][:, :3].astype(np.float64) - o.vel[:, :3].astype(np.float64))) <= tol
+    # fused steps from a common state
+    st = g.get_state(); e = g.get_embedded()
+    for x in (g, o):
+        x.set_state(st["pos"], st["vel"], st["tag"], step=1)
+    g.set_embedded(e["pos"], e["vel"], bm, 12, K, R0, NSUB); o.emb["pos"][:] = e["pos"]; o.emb["vel"][:] = e["vel"]
+    g.step(3); o.step(3)
+    s = g.get_state(); e = g.get_embedded()
+    a, b = np.argsort(s["tag"]), np.argsort(o.tag)
+    tol3 = 1e-10 if dtype == np.float64 else 1e-4
+    assert np.max(np.abs(s["vel"][a][:, :3].astype(np.float64) - o.vel[b][:, :3].astype(np.float64))) <= tol3
+    assert np.max(np.abs(e["vel"] - o.emb["vel"])) <= tol3 and np.max(np.abs(e["pos"] - o.emb["pos"])) <= tol3
+    assert np.array_equal(e["cell"], o.emb["cell"]) and np.array_equal(s["cell"][a], o.cell[b])
+    g.close()
+
+
+def test_thermostat_cools_hot_beads_and_solvent_to_kT():
+    """Equipartition under the thermostat: solvent at 1.8 kT and beads at 4 kT both end at the thermostat's kT."""
+    from paper_1801_10187_b200 import MPCD
+    n, M = (24, 24, 24), 5
+    pos, vel, tag = synth.solvent(n, M, seed=80, kT=1.8, dtype=np.float32)
+    bp, bv, bm = synth.chains(n, 200, 20, seed=81, kT=4.0, mass=MB, r0=R0)
+    g = MPCD([float(x) for x in n], pos.shape[0], kT=1.0, seed=80, init_state=False, thermostat=True)
+    g.set_state(pos, vel, tag); g.set_embedded(bp, bv, bm, 20, K, R0, NSUB)
+    P0 = vel[:, :3].astype(np.float64).sum(axis=0) + (bm[:, None] * bv).sum(axis=0)
+    g.step(100)
+    kb, ks = [], []
+    for _ in range(20):
+        g.step(5)
+        kb.append((bm[:, None] * g.get_embedded()["vel"] ** 2).sum() / (3 * bm.size))
+        ks.append((g.get_state(pos=False, tag=False, cell=False)["vel"][:, :3].astype(np.float64) ** 2).sum() / (3 * pos.shape[0]))
+    assert abs(np.mean(ks) - 1.0) < 0.01 and abs(np.mean(kb) - 1.0) < 0.04, (np.mean(ks), np.mean(kb))
+    P1 = g.get_state(pos=False, tag=False, cell=False)["vel"][:, :3].astype(np.float64).sum(axis=0) + (bm[:, None] * g.get_embedded()["vel"]).sum(axis=0)
+    assert np.max(np.abs(P1 - P0)) / (pos.shape[0] + MB * bm.size) <= 1e-6
+    g.close()
+
+
 def test_embedded_argument_checks():
     from paper_1801_10187_b200 import MPCD, MPCDError
     bp, bv, bm = synth.chains((4, 4, 4), 2, 5, seed=1)
-    for kw in (dict(rule="at"), dict(thermostat=True)):
+    for kw in (dict(rule="at"), dict(deterministic=True)):
         g = MPCD([4.0] * 3, 320, seed=1, **kw)
         with pytest.raises(MPCDError) as err:
             g.set_embedded(bp, bv, bm, 5, K, R0, NSUB)

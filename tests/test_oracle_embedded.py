@@ -123,3 +123,94 @@ def test_hot_beads_relax_to_the_solvent_temperature(oracle):
     kT_solvent = (o.vel[:, :3] ** 2).sum() / (3 * pos.shape[0])
     assert abs(np.mean(samples) - kT_solvent) < 0.06, (np.mean(samples), kT_solvent)
     assert 1.0 < kT_solvent < 1.2
+
+
+# ---- thermostat with embedded beads (reading A28; PAPER.md:47 eq. 3, :157, :159) ----
+
+def _thermo_pair(oracle, dtype, seed=31, kT_beads=3.0):
+    n = (7, 6, 5); M = 6
+    pos, vel, tag = synth.solvent(n, M, seed=seed, kT=1.6, dtype=dtype)
+    bp, bv, bm = synth.chains(n, 9, 8, seed=seed + 1, kT=kT_beads)
+    o = oracle.OracleMPCD([float(x) for x in n], pos.shape[0], kT=1.0, seed=seed, dtype=dtype, init=False, sort_period=0, thermostat=True)
+    o.set_state(pos, vel, tag); o.set_embedded(bp, bv, bm, 8, 1000.0, 0.5, 10)
+    return o, bm
+
+
+def test_bead_rotation_with_xi_reduces_to_the_plain_one_and_scales_the_relative_velocity(oracle):
+    rng = np.random.default_rng(5)
+    nb, Nc = 40, 12
+    cell = rng.integers(0, Nc, nb).astype(np.int32)
+    u = rng.standard_normal((Nc, 3)); axis = oracle.draw_axis(9, 4, Nc)
+    v0 = rng.standard_normal((nb, 3))
+    a = v0.copy(); b = v0.copy(); c = v0.copy()
+    oracle.collide_srd_beads(a, cell, u, axis, 2.2)
+    oracle.collide_srd_beads_xi(b, cell, u, axis, np.ones(Nc), 2.2)
+    np.testing.assert_allclose(a, b, rtol=0, atol=1e-14)               # xi = 1: the pinned plain rotation (sense, angle) up to the order of the additions
+    oracle.collide_srd_beads_xi(c, cell, u, axis, np.full(Nc, 2.0), 2.2)
+    np.testing.assert_allclose(c - u[cell], 2.0 * (a - u[cell]), rtol=0, atol=1e-14)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_cell_energy_with_beads_is_the_sum_over_all_particles_of_the_cell(oracle, dtype):
+    o, bm = _thermo_pair(oracle, dtype)
+    o.stream(); o.shift_and_bin()
+    Nc = o.Nc
+    vs = o.vel[:, :3].astype(np.float64); vb = o.emb["vel"]; cs = o.cell; cb = o.emb["cell"]
+    P = np.stack([np.bincount(cs, o.m * vs[:, d], Nc) + np.bincount(cb, bm * vb[:, d], Nc) for d in range(3)], axis=1)
+    Mc = np.bincount(cs, None, Nc) * o.m + np.bincount(cb, bm, Nc)
+    u = np.where(Mc[:, None] > 0, P / np.maximum(Mc, 1e-300)[:, None], 0.0)
+    E = np.bincount(cs, 0.5 * o.m * ((vs - u[cs]) ** 2).sum(axis=1), Nc) + np.bincount(cb, 0.5 * bm * ((vb - u[cb]) ** 2).sum(axis=1), Nc)
+    np.testing.assert_allclose(o.erel_tot, E, rtol=1e-12, atol=1e-13)
+    assert np.array_equal(o.ntot, np.bincount(cs, None, Nc) + np.bincount(cb, None, Nc))
+    # no beads: the same routine about u = S / N_c is the pinned two-pass E_rel of oracle_finalize, bit for bit
+    erel, ntot = oracle.erel_with_beads(o.vel, o.cell, o.m, o.count, oracle.finalize_cells(o.vel, o.cell, Nc, o.m, o.count, o.sumv)[0],
+                                        np.zeros(0, np.int32), np.zeros((0, 3)), np.zeros(0))
+    assert np.array_equal(erel, oracle.finalize_cells(o.vel, o.cell, Nc, o.m, o.count, o.sumv)[1]) and np.array_equal(ntot, o.count)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_thermostatted_collision_with_beads_sets_every_cell_to_its_drawn_energy(oracle, dtype):
+    """xi^2 E_k = E^ over solvent and beads together, the cell's momentum (incl. the beads) kept; cells with fewer than two
+    particles untouched; the drawn energies follow the cell's particle count incl. beads."""
+    o, bm = _thermo_pair(oracle, dtype)
+    o.stream(); o.shift_and_bin()
+    Nc = o.Nc
+    cs, cb = o.cell.copy(), o.emb["cell"].copy()
+    def moments():
+        vs = o.vel[:, :3].astype(np.float64); vb = o.emb["vel"]
+        P = np.stack([np.bincount(cs, o.m * vs[:, d], Nc) + np.bincount(cb, bm * vb[:, d], Nc) for d in range(3)], axis=1)
+        E = np.bincount(cs, 0.5 * o.m * ((vs - o.u[cs]) ** 2).sum(axis=1), Nc) + np.bincount(cb, 0.5 * bm * ((vb - o.u[cb]) ** 2).sum(axis=1), Nc)
+        return P, E
+    P0, E0 = moments()
+    ehat, xi, ntot = o.ehat.copy(), o.xi.copy(), o.ntot.copy()
+    v_before, b_before = o.vel.copy(), o.emb["vel"].copy()
+    o.collide_srd()
+    P1, E1 = moments()
+    tol = 1e-12 if dtype == np.float64 else 3e-6
+    np.testing.assert_allclose(P1, P0, atol=30 * tol)
+    live = (ntot >= 2) & (E0 > 0)
+    np.testing.assert_allclose(E1[live], ehat[live], rtol=30 * tol)
+    assert np.all(xi[~live] == 1.0)
+    lone = ntot < 2
+    assert np.array_equal(o.vel[np.isin(cs, np.flatnonzero(lone))], v_before[np.isin(cs, np.flatnonzero(lone))])
+    np.testing.assert_allclose(o.emb["vel"][np.isin(cb, np.flatnonzero(lone))], b_before[np.isin(cb, np.flatnonzero(lone))], atol=1e-14)
+    # E^ ~ Gamma(3 (n - 1) / 2, kT): its mean over cells of n particles is 1.5 (n - 1) kT
+    sel = ntot >= 2
+    assert abs(ehat[sel].sum() / (1.5 * (ntot[sel] - 1)).sum() - 1.0) < 5.0 / math.sqrt(1.5 * (ntot[sel] - 1).sum())
+
+
+@pytest.mark.slow
+def test_thermostat_brings_solvent_and_hot_beads_to_kT(oracle):
+    n = (9, 9, 9); M = 5
+    pos, vel, tag = synth.solvent(n, M, seed=61, kT=1.8, dtype=np.float64)
+    bp, bv, bm = synth.chains(n, 25, 10, seed=62, kT=4.0)
+    o = oracle.OracleMPCD([float(x) for x in n], pos.shape[0], kT=1.0, seed=61, dtype=np.float64, init=False, sort_period=0, thermostat=True)
+    o.set_state(pos, vel, tag); o.set_embedded(bp, bv, bm, 10, 1000.0, 0.5, 10)
+    o.step(60)
+    kb, ks = [], []
+    for _ in range(40):
+        o.step(3)
+        kb.append((bm[:, None] * o.emb["vel"] ** 2).sum() / (3 * bm.size))
+        ks.append((o.vel[:, :3] ** 2).sum() / (3 * pos.shape[0]))
+    assert abs(np.mean(ks) - 1.0) < 0.03, np.mean(ks)                 # canonical: <m v^2> = kT (the cell means carry their share)
+    assert abs(np.mean(kb) - 1.0) < 0.08, np.mean(kb)                 # equipartition of the beads at the thermostat's kT
