@@ -4,6 +4,7 @@
 // draw (a2) and cos/sin of the SRD angle (A15).
 #include "../../include/mpcd.h"
 #include "mpcd_brick.cuh"
+#include "mpcd_small.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -43,6 +44,9 @@ struct mpcd {
     double *qacc[2] = {nullptr, nullptr};     // sum |v|^2 per cell
     double *at_acc[2] = {nullptr, nullptr};   // {Dx, Dy, Dz, -} per cell (AT only, allocated on first use)
     double *axis[2] = {nullptr, nullptr};     // {nx, ny, nz, -} per cell
+    // small systems (mpcd_small.cuh): a third accumulator set, allocated on first use; whether the cooperative kernel may be used
+    double *acc_x = nullptr, *qacc_x = nullptr;
+    bool small_ok = true;
     // embedded solute (NEXT-1; mpcd_embedded.cuh): beads in double, their per-cell sums by step parity
     int64_t emb_n = 0;
     int32_t emb_chain_len = 0, emb_nsub = 0;
@@ -520,6 +524,78 @@ int emb_join_stream(mpcd_t *h)
     return MPCD_OK;
 }
 
+// Small systems: `n` consecutive fused steps (collide t .. t + n - 1, none of them a sort step) as ONE cooperative launch
+// (mpcd_small.cuh).  Returns MPCD_OK with *done = false when the system is not eligible (too large for one resident wave,
+// another rule, thermostat, beads, brick order, profiling): the caller then takes the ordinary per-step path.
+template <typename T, unsigned F> int small_launch_t(mpcd_t *h, const PassArgs<T> &a, const SmallArgs &sa, bool *done)
+{
+    static int capacity = -1;                        // blocks of one resident wave, per instantiation
+    if (capacity < 0) {
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_steps<T, F>, kPassThreads, 0) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+        capacity = per_sm * h->num_sms;
+    }
+    const unsigned grid = grid_for(h->N, kPassThreads);
+    if ((int64_t)grid > (int64_t)capacity) return MPCD_OK;
+    void *args[2] = {const_cast<PassArgs<T> *>(&a), const_cast<SmallArgs *>(&sa)};
+    if (cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(small_steps<T, F>), dim3(grid), dim3(kPassThreads), args, 0, h->stream) != cudaSuccess) {
+        cudaGetLastError();                          // no cooperative launch on this device / context: never try again
+        h->small_ok = false;
+        return MPCD_OK;
+    }
+    *done = true;
+    return MPCD_OK;
+}
+
+int small_run(mpcd_t *h, int set, uint64_t t, int32_t n, unsigned fe, bool *done)
+{
+    *done = false;
+    if (!h->small_ok || h->profiling || h->debug_sync || h->opt.rule != MPCD_SRD || thermostatted(h) || embedded(h) || h->grid.on) return MPCD_OK;
+    if (h->N > (int64_t)h->num_sms * 16 * kPassThreads) return MPCD_OK;              // cannot be one resident wave whatever the kernel
+    if (!h->acc_x) {
+        int rc = dev_alloc_t(h, &h->acc_x, (size_t)h->Nc * 4);
+        if (!rc) rc = dev_alloc_t(h, &h->qacc_x, (size_t)h->Nc);
+        if (rc) return rc;
+    }
+    const int nxt = set ^ 1;
+    int rc = zero_set(h, nxt, true, false);          // the set phase 0 accumulates into; the kernel zeroes the later ones itself
+    if (rc) return rc;
+    PassPlan pl;
+    pl.cset = set; pl.bset = nxt;
+    pl.step_collide = t; pl.step_bin = t + 1;
+    pl.alpha = h->opt.alpha;
+    SmallArgs sa{};
+    sa.acc3[0] = h->acc[set]; sa.acc3[1] = h->acc[nxt]; sa.acc3[2] = h->acc_x;
+    sa.qacc3[0] = h->qacc[set]; sa.qacc3[1] = h->qacc[nxt]; sa.qacc3[2] = h->qacc_x;
+    sa.axis2[0] = h->axis[0]; sa.axis2[1] = h->axis[1];
+    const int out = (int)((t + (uint64_t)n) & 1);
+    sa.acc_out = h->acc[out]; sa.qacc_out = h->qacc[out];
+    sa.t0 = t; sa.nphases = n; sa.a_cell = h->a;
+    const unsigned F = kSRD | kStream | kBin | fe | fixed_flag(h);
+    if (h->opt.precision == MPCD_FP64) {
+        const PassArgs<double> a = make_args<double>(h, pl);
+        if (F & kEnergy) rc = small_launch_t<double, kSRD | kStream | kBin | kEnergy>(h, a, sa, done);
+        else rc = small_launch_t<double, kSRD | kStream | kBin>(h, a, sa, done);
+    } else {
+        const PassArgs<float> a = make_args<float>(h, pl);
+        switch (F) {
+            case kSRD | kStream | kBin: rc = small_launch_t<float, kSRD | kStream | kBin>(h, a, sa, done); break;
+            case kSRD | kStream | kBin | kEnergy: rc = small_launch_t<float, kSRD | kStream | kBin | kEnergy>(h, a, sa, done); break;
+            case kSRD | kStream | kBin | kFixed: rc = small_launch_t<float, kSRD | kStream | kBin | kFixed>(h, a, sa, done); break;
+            case kSRD | kStream | kBin | kEnergy | kFixed: rc = small_launch_t<float, kSRD | kStream | kBin | kEnergy | kFixed>(h, a, sa, done); break;
+            default: break;
+        }
+    }
+    if (rc || !*done) return rc;
+    LAUNCH_CHECK(h);
+    // cell-array state after n phases: the sums of step t + n are complete in set (t + n) & 1, the axes of steps t + n and
+    // t + n - 1 in their parities; every other set is dirty
+    h->zeroed[0] = h->zeroed[1] = false;
+    h->xi_valid[0] = h->xi_valid[1] = false;
+    for (uint64_t u = t + (uint64_t)n - 1; u <= t + (uint64_t)n; ++u) { h->axis_valid[u & 1] = true; h->axis_step[u & 1] = u; }
+    return MPCD_OK;
+}
+
 // a8, first half: exclusive scan of the per-cell counts of accumulator set `s` in sort-key order -> cell_start (the
 // write cursors) and, in brick-major order, the segment starts of the order being prepared (brick_start[bcur ^ 1])
 int scan_counts(mpcd_t *h, int s)
@@ -723,6 +799,7 @@ int mpcd_create_ex(mpcd_t **out, const double box[3], int64_t N, double a, doubl
         h->nbricks = g.on ? g.nb[0] * g.nb[1] * g.nb[2] : 0;
     }
     if (const char *e = std::getenv("MPCD_DEBUG_SYNC")) h->debug_sync = std::atoi(e) != 0;
+    if (const char *e = std::getenv("MPCD_NO_COOP")) h->small_ok = std::atoi(e) == 0;      // A/B timing of the small-system kernel
     {
         int dev = 0, sms = 0;
         if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) h->num_sms = sms;
@@ -872,6 +949,18 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     // steady state, two launches per step: cell_prepare (zeroed set and axes of step t + 1), then collide(t) fused with
     // stream + bin + accumulate (t + 1)
     for (int32_t j = 1; j < nsteps; ++j) {
+        if (!at && !sort_pending && nsteps - j >= 2) {     // small systems: the run of steps up to the next sort in one cooperative launch
+            int32_t run = 1;
+            while (j + run < nsteps && !sort_due(h, t + (uint64_t)run)) ++run;
+            bool done = false;
+            if (run >= 2) { rc = small_run(h, set, t, run, fe, &done); if (rc) return rc; }
+            if (done) {
+                t += (uint64_t)run; set = (int)(t & 1); j += run - 1;
+                shift_for(h, t, pl.shift);                 // the shift of the last bin (mpcd_get_shift)
+                sort_pending = sort_due(h, t);
+                continue;
+            }
+        }
         const int nxt = set ^ 1;
         rc = prepare(h, nxt, true, false, !at, t + 1);
         if (rc) return rc;

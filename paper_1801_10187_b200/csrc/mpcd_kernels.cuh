@@ -21,6 +21,8 @@
 //                    (mpcd_embedded.cuh)
 //   kFixed    a4     deterministic accumulation: the cell sums are 64-bit fixed-point integers (mpcd_device.cuh), both
 //                    where they are accumulated (kBin) and where they are read (kSRD)
+//   kCoherent        the cell arrays read by kSRD were written earlier in the SAME launch (mpcd_small.cuh): plain loads ordered
+//                    by the grid barrier instead of the read-only (.nc) path, which promises data constant for the whole launch
 //   kSortOut  a8     sort by cell on the way out: instead of in place, the particle is written
 //                    to slot cell_start[c] + (atomic cursor) of the duplicate arrays, c = its cell in the step
 //                    being collided; the separate read-and-scatter pass of the sort disappears
@@ -36,7 +38,7 @@
 
 namespace mpcdk {
 
-enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u, kEmbedded = 512u, kFixed = 1024u };
+enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u, kEmbedded = 512u, kFixed = 1024u, kCoherent = 2048u };
 
 template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
@@ -97,13 +99,16 @@ __device__ __forceinline__ int w_to_cell(double w) { return (int)__double_as_lon
 #ifndef MPCD_MINBLOCKS_F64
 #define MPCD_MINBLOCKS_F64 10
 #endif
+template <unsigned F> struct PassScratch {
+    using type = typename std::conditional<(F & kBin) && (F & kATDraw) && !(F & kATStored), WarpScratchX, WarpScratch>::type;
+    static constexpr int count = (F & (kBin | kATDraw)) ? kPassThreads / 32 : 1;     // one per warp when the pass accumulates
+};
+
+// The pass over one particle per thread (particle i = blockIdx.x * kPassThreads + threadIdx.x); `w` is the warp's scratch.
 template <typename T, unsigned F>
-__global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_F32 : MPCD_MINBLOCKS_F64) particle_pass(const PassArgs<T> a)
+__device__ __forceinline__ void pass_body(const PassArgs<T> &a, typename PassScratch<F>::type &w)
 {
     using V4 = typename Vec4<T>::type;
-    using WS = typename std::conditional<(F & kBin) && (F & kATDraw) && !(F & kATStored), WarpScratchX, WarpScratch>::type;
-    __shared__ WS ws[(F & (kBin | kATDraw)) ? kPassThreads / 32 : 1];
-    WS &w = ws[(F & (kBin | kATDraw)) ? (threadIdx.x >> 5) : 0];
     const int64_t i = (int64_t)blockIdx.x * kPassThreads + threadIdx.x;
     const bool valid = i < a.N;
     const int inactive = -1 - (int)(threadIdx.x & 31);
@@ -120,8 +125,8 @@ __global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_
     if ((F & kSortOut) && valid) o = atomicAdd(a.cursor + c, 1); // issued early: its latency hides behind the gather
     if (F & kSRD) {
         {
-            f64x4 s = ld256_nc(a.sums + 4 * (size_t)c);          // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
-            const f64x4 n = ld256_nc(a.axis + 4 * (size_t)c);
+            f64x4 s = (F & kCoherent) ? ld256(a.sums + 4 * (size_t)c) : ld256_nc(a.sums + 4 * (size_t)c);   // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
+            const f64x4 n = (F & kCoherent) ? ld256(a.axis + 4 * (size_t)c) : ld256_nc(a.axis + 4 * (size_t)c);
             if (F & kFixed) { s.x = acc_value(s.x, true); s.y = acc_value(s.y, true); s.z = acc_value(s.z, true); s.w = acc_count(s.w, true); }
             double ux, uy, uz;
             if (F & kEmbedded) {
@@ -185,6 +190,13 @@ __global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_
         warp_cell_accumulate<T, true, (F & kEnergy) != 0, false, true>(a.acc, a.qacc, w, c, v.x, v.y, v.z, a.at_acc, ex, ey, ez);
     else if constexpr ((F & kBin) != 0) warp_cell_accumulate<T, true, (F & kEnergy) != 0, (F & kFixed) != 0>(a.acc, a.qacc, w, c, v.x, v.y, v.z);
     else if constexpr ((F & kATDraw) != 0) warp_cell_accumulate<double, false, false>(a.at_acc, nullptr, w, c, ex, ey, ez);
+}
+
+template <typename T, unsigned F>
+__global__ void __launch_bounds__(kPassThreads, sizeof(T) == 4 ? MPCD_MINBLOCKS_F32 : MPCD_MINBLOCKS_F64) particle_pass(const PassArgs<T> a)
+{
+    __shared__ typename PassScratch<F>::type ws[PassScratch<F>::count];
+    pass_body<T, F>(a, ws[PassScratch<F>::count > 1 ? (threadIdx.x >> 5) : 0]);
 }
 
 // Cell index of every particle (the cache in vel.w) as an int32 array, on demand (mpcd_get_state, mpcd_device_ptrs).
