@@ -64,16 +64,16 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def csrc_hash() -> str:
-    """sha256 (first 16 hex digits) over the kernel sources, in name order: what an ncu capture is stamped with."""
+def csrc_hash(brick: int = 0) -> str:
+    """sha256 (first 16 hex digits) over the sources of the step kernel, in name order: what an ncu capture is stamped with
+    (the per-particle kernel lives in mpcd_device.cuh, mpcd_embedded.cuh and mpcd_kernels.cuh; the brick kernel adds mpcd_brick.cuh)."""
     import hashlib
     d = os.path.join(ROOT, "paper_1801_10187_b200", "csrc")
     h = hashlib.sha256()
-    for name in sorted(os.listdir(d)):
-        if name.endswith((".cu", ".cuh")):
-            h.update(name.encode())
-            with open(os.path.join(d, name), "rb") as f:
-                h.update(f.read())
+    for name in ["mpcd_brick.cuh"] * int(bool(brick)) + ["mpcd_device.cuh", "mpcd_embedded.cuh", "mpcd_kernels.cuh"]:
+        h.update(name.encode())
+        with open(os.path.join(d, name), "rb") as f:
+            h.update(f.read())
     return h.hexdigest()[:16]
 
 
@@ -92,8 +92,8 @@ def ncu_traffic(workload: str, precision: str, brick: int):
         pass
     if found is None:
         return None, "no ncu capture committed for this workload"
-    if found[1] != csrc_hash():
-        return None, f"ncu capture is of kernel sources {found[1]}, the tree is {csrc_hash()}: not quoted"
+    if found[1] != csrc_hash(brick):
+        return None, f"ncu capture is of kernel sources {found[1]}, the tree is {csrc_hash(brick)}: not quoted"
     return found[0], f"ncu --set full capture of kernel sources {found[1]} (profiles/ncu_traffic.csv)"
 
 

@@ -41,6 +41,12 @@ namespace mpcdk {
 #ifndef MPCD_BRICK_MINBLOCKS
 #define MPCD_BRICK_MINBLOCKS 8
 #endif
+// MPCD_BRICK_SUMS = 0 keeps the window read but accumulates like the per-particle kernel (match.any, shuffle tree, transposed
+// RED): measured slower than both (DESIGN.md 5.1 probe table), kept as a compile-time probe.
+#ifndef MPCD_BRICK_SUMS
+#define MPCD_BRICK_SUMS 1
+#endif
+constexpr bool kWinSums = MPCD_BRICK_SUMS != 0;      // 1: the next step's sums in the shared-memory window; 0: in-warp aggregation + global RED (the per-particle kernel's route)
 constexpr int kBrickThreads = MPCD_BRICK_THREADS;
 constexpr int kFlushLimit = 2048;      // additions per window cell between two flushes that the fixed-point headroom allows
 
@@ -77,7 +83,7 @@ __device__ __forceinline__ int wrap(int v, int n)
 template <unsigned F> struct BrickSmem {
     static constexpr int NV = (F & kEnergy) ? 4 : 3;            // fixed-point sums per cell: Sx, Sy, Sz [, sum |v|^2]
     static constexpr int NA = (F & kThermo) ? 4 : 3;            // axis [, xi]
-    static constexpr size_t bytes = (size_t)kW * (8 * (3 + NA) + 4 * (2 * NV + 2));
+    static constexpr size_t bytes = kWinSums ? (size_t)kW * (8 * (3 + NA) + 4 * (2 * NV + 2)) : (size_t)kW * 8 * (3 + NA);
 };
 
 // Thread -> particle mapping.  A warp's 32 lanes are four QUARTERS of 8 lanes; quarter k of the CTA streams through its
@@ -100,6 +106,7 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
     unsigned (*sHi)[kW] = sLo + NV;                                                  // [NV][kW]
     unsigned *sCnt = reinterpret_cast<unsigned *>(sHi + NV);                         // [kW]
     int *sCell = reinterpret_cast<int *>(sCnt + kW);                                 // [kW]     global cell of every slot of that window
+    __shared__ WarpScratch wscr[kWinSums ? 1 : kBrickThreads / 32];
     const int tid = threadIdx.x;
     const int b = blockIdx.x;
     const int lo = g.brick_start[b], hi = g.brick_start[b + 1];
@@ -141,14 +148,16 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
         sU[0][w] = ux; sU[1][w] = uy; sU[2][w] = uz;
         sA[0][w] = n.x; sA[1][w] = n.y; sA[2][w] = n.z;
         if (kTh) sA[NA - 1][w] = n.w;
+        if (kWinSums) {
 #pragma unroll
-        for (int k = 0; k < NV; ++k) { sLo[k][w] = 0u; sHi[k][w] = 0u; }
-        sCnt[w] = 0u;
-        cx = ax0 + lx; cy = ay0 + ly; cz = az0 + lz;
-        while (cx >= n0) cx -= n0;
-        while (cy >= n1) cy -= n1;
-        while (cz >= n2) cz -= n2;
-        sCell[w] = cx + n0 * (cy + n1 * cz);
+            for (int k = 0; k < NV; ++k) { sLo[k][w] = 0u; sHi[k][w] = 0u; }
+            sCnt[w] = 0u;
+            cx = ax0 + lx; cy = ay0 + ly; cz = az0 + lz;
+            while (cx >= n0) cx -= n0;
+            while (cy >= n1) cy -= n1;
+            while (cz >= n2) cz -= n2;
+            sCell[w] = cx + n0 * (cy + n1 * cz);
+        }
     }
     __syncthreads();
 
@@ -179,7 +188,7 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
     const int off0 = rot * kW, off1 = ((rot + 1) % NV) * kW, off2 = ((rot + 2) % NV) * kW, off3 = ((rot + 3) % NV) * kW;
     int since = 0;
     for (int j = 0; j < m; ++j, i += 8) {
-        if (since + kBrickThreads > kFlushLimit) {
+        if (kWinSums && since + kBrickThreads > kFlushLimit) {
             __syncthreads();
             flush();
             __syncthreads();
@@ -248,6 +257,10 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
         if (valid) {
             store4((kSo ? a.vel_out : a.vel) + o, v);
             if (kSo) a.tag_out[o] = tag;
+        }
+        if constexpr (!kWinSums) {       // the per-particle kernel's accumulation: match.any, shuffle tree, transposed fp64 RED (mpcd_device.cuh)
+            warp_cell_accumulate<T, true, kE, kFx>(a.acc, a.qacc, wscr[tid >> 5], valid ? cn : -1 - (tid & 31), v.x, v.y, v.z);
+        } else if (valid) {
             const double dx = (double)v.x, dy = (double)v.y, dz = (double)v.z;
             const double q = kE ? sq_norm(dx, dy, dz) : 0.0;
             int lx = jx - ax0, ly = jy - ay0, lz = jz - az0;
@@ -287,8 +300,10 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
             }
         }
     }
-    __syncthreads();
-    flush();
+    if (kWinSums) {
+        __syncthreads();
+        flush();
+    }
 }
 
 }  // namespace mpcdk

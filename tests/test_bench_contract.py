@@ -50,5 +50,5 @@ def test_ncu_traffic_is_only_quoted_for_the_kernel_sources_it_was_taken_on():
     for row in open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")).read().splitlines()[1:]:
         w = [x.strip() for x in row.split(",")]
         value, note = bench.ncu_traffic(w[0], w[1], int(w[2]))
-        assert (value is not None) == (w[4] == bench.csrc_hash()), note
+        assert (value is not None) == (w[4] == bench.csrc_hash(int(w[2]))), note
     assert bench.ncu_traffic("C1", "mixed", 0) == (None, "no ncu capture committed for this workload")
