@@ -83,3 +83,19 @@ def test_small_path_is_left_alone_by_other_rules_and_options(oracle):
         a, b = np.argsort(s["tag"]), np.argsort(o.tag)
         explained_compare(s["pos"][a], s["vel"][a], s["cell"][a], o.pos[b], o.vel[b], o.cell[b], g.get_shift(), 1.0, [8.0] * 3, 1e-4, np.float32, pos_ulps=4)
         g.close()
+
+
+def test_config1_thousand_steps_keep_momentum_and_energy():
+    """BASELINE config 1 for 1000 steps, 40 cooperative launches: momentum drift <= 1e-6 (A25), energy to fp32 store rounding."""
+    cfg = synth.CONFIGS["C1"]
+    g, (pos, vel, tag) = _gpu(cfg["n"], cfg["M"], cfg["seed"], np.float32)
+    N = pos.shape[0]
+    P0, KE0, _ = g.get_thermo()
+    g.step(1000)
+    P, KE, kT = g.get_thermo()
+    assert g.stats()["step"] == 1000 and g.stats()["sorts"] == 40 and g.stats()["kernel_launches"] < 400
+    assert float(np.max(np.abs(np.asarray(P) - np.asarray(P0)))) / N <= 1e-6
+    assert abs(KE - KE0) / KE0 <= 1e-4
+    s = g.get_state()
+    assert np.array_equal(np.sort(s["tag"]), tag) and np.all((s["pos"][:, :3] >= 0) & (s["pos"][:, :3] < 8.0))
+    g.close()
