@@ -117,11 +117,18 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
     const int gx0 = wrap(bx * kBX + g.og[0], n0), gy0 = wrap(by * kBY + g.og[1], n1), gz0 = wrap(bz * kBZ + g.og[2], n2);
     const int ax0 = wrap(bx * kBX + g.oa[0], n0), ay0 = wrap(by * kBY + g.oa[1], n1), az0 = wrap(bz * kBZ + g.oa[2], n2);
 
-    // quarter k streams blocks [k m, (k + 1) m) of 8 particles, counted from the 128-byte line the segment starts in
+    // The segment is cut in blocks of 8 particles (one 128-byte line of float4), counted from the line it starts in, and the
+    // blocks are dealt to the 16 quarters in contiguous, BALANCED runs: the first nblk mod 16 quarters stream one block more
+    // than the others.  All quarters are busy for the same number of iterations but the last, in which the idle quarters are
+    // the high ones: they fill whole warps, which skip the body.
     const int a0 = lo & ~7;
     const int nblk = (hi - a0 + 7) >> 3;
-    const int m = (nblk + kBrickThreads / 8 - 1) / (kBrickThreads / 8);
-    int i = a0 + 8 * (tid >> 3) * m + (tid & 7);
+    constexpr int kQuarters = kBrickThreads / 8;
+    const int mlo = nblk / kQuarters, mrem = nblk - mlo * kQuarters;
+    const int m = mlo + (mrem > 0);                      // iterations of the CTA
+    const int quarter = tid >> 3;
+    const int mine = mlo + (quarter < mrem);             // blocks of this quarter
+    int i = a0 + 8 * (quarter * mlo + (quarter < mrem ? quarter : mrem)) + (tid & 7);
     auto clamped = [&](int idx) { return idx < lo ? lo : (idx >= hi ? hi - 1 : idx); };
     V4 vn = load4(a.vel + clamped(i));                  // the first block's loads are in flight while the window is built
     V4 pn = load4(a.pos + clamped(i));
@@ -201,12 +208,13 @@ __global__ void __launch_bounds__(kBrickThreads, MPCD_BRICK_MINBLOCKS) brick_pas
             since = 0;
         }
         since += kBrickThreads;
-        const bool valid = i >= lo && i < hi;            // other lanes work on a copy of a particle of the segment and store nothing
+        const bool valid = j < mine && i >= lo && i < hi;   // other lanes work on a copy of a particle of the segment and store nothing
         V4 v = vn, p = pn;
-        if (j + 1 < m) {                                 // the next block's loads fly during this block's arithmetic
+        if (j + 1 < mine) {                              // the next block's loads fly during this block's arithmetic
             vn = load4(a.vel + clamped(i + 8));
             pn = load4(a.pos + clamped(i + 8));
         }
+        if (!__any_sync(0xffffffffu, j < mine)) continue;   // a warp whose four quarters are done (last iteration only)
         uint32_t tag = 0;
         if (kSo) tag = a.tag[clamped(i)];
         const int c = w_to_cell(v.w);                    // cell of the step being collided
