@@ -552,6 +552,7 @@ int small_run(mpcd_t *h, int set, uint64_t t, int32_t n, unsigned fe, bool *done
     *done = false;
     if (!h->small_ok || h->profiling || h->debug_sync || h->opt.rule != MPCD_SRD || thermostatted(h) || embedded(h) || h->grid.on) return MPCD_OK;
     if (h->N > (int64_t)h->num_sms * 16 * kPassThreads) return MPCD_OK;              // cannot be one resident wave whatever the kernel
+    if (h->Nc > 4 * (int64_t)grid_for(h->N, kPassThreads) * kPassThreads) return MPCD_OK;   // a dilute box: the cell side (an fp64 sincos per cell) would dominate the phase
     if (!h->acc_x) {
         int rc = dev_alloc_t(h, &h->acc_x, (size_t)h->Nc * 4);
         if (!rc) rc = dev_alloc_t(h, &h->qacc_x, (size_t)h->Nc);
