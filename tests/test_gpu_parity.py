@@ -280,3 +280,25 @@ def test_device_init_has_the_papers_initial_condition(oracle):
         po, vo, _ = oracle.init_state(11, 80000, [20.0] * 3, math.sqrt(kT / m), dtype)
         assert np.array_equal(s["pos"][:, :3], po[:, :3])
         np.testing.assert_allclose(v, vo[:, :3].astype(np.float64), rtol=0, atol=1e-6 if dtype == np.float32 else 1e-13)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_at_fused_kernel_teacher_forced(oracle, dtype):
+    """The AT rule inside mpcd_step (kATStored: the drawn dv rides in vel.xyz between two launches and a cell's ONE accumulator
+    holds sum(v) - sum(dv), eq. 4): every two steps the oracle restarts from the GPU's state and must land on the
+    GPU's state two steps later at the plain north_star tolerance, every mismatch explained; a sort every 3 steps."""
+    n = (12, 10, 9)
+    g, o = _pair(oracle, n, 5, 17, dtype, rule="at", sort_period=3)
+    box = [float(x) for x in n]
+    for t in range(0, 12, 2):
+        st = g.get_state()
+        o.set_state(st["pos"], st["vel"], st["tag"], step=t)
+        g.step(2); o.step(2)
+        gs = _by_tag(g.get_state())
+        os_ = np.argsort(o.tag)
+        r = explained_compare(gs["pos"], gs["vel"], gs["cell"], o.pos[os_], o.vel[os_], o.cell[os_], g.get_shift(), 1.0, box, _tol(dtype), dtype,
+                              pos_ulps=2 if dtype == np.float32 else 300)
+        assert r["bad_cell"] <= (1 if dtype == np.float32 else 0), (t, r)
+        # eq. 4 conserves every cell's momentum: so does the whole box, to rounding
+        assert np.max(np.abs(gs["vel"][:, :3].astype(np.float64).sum(axis=0) - st["vel"][:, :3].astype(np.float64).sum(axis=0))) <= (1e-9 if dtype == np.float64 else 2e-3)
+    g.close()
