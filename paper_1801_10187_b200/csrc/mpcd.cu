@@ -524,6 +524,8 @@ int emb_join_stream(mpcd_t *h)
     return MPCD_OK;
 }
 
+inline bool sort_due(const mpcd_t *h, uint64_t t) { return h->opt.sort_period > 0 && (t % (uint64_t)h->opt.sort_period) == 0; }
+
 // Small systems: `n` consecutive fused steps (collide t .. t + n - 1, none of them a sort step) as ONE cooperative launch
 // (mpcd_small.cuh).  Returns MPCD_OK with *done = false when the system is not eligible (too large for one resident wave,
 // another rule, thermostat, beads, brick order, profiling): the caller then takes the ordinary per-step path.
@@ -572,6 +574,12 @@ int small_run(mpcd_t *h, int set, uint64_t t, int32_t n, unsigned fe, bool *done
     const int out = (int)((t + (uint64_t)n) & 1);
     sa.acc_out = h->acc[out]; sa.qacc_out = h->qacc[out];
     sa.t0 = t; sa.nphases = n; sa.a_cell = h->a;
+    int32_t nsorts = 0, first_sort = n;              // sorts inside the launch (few cells only; else the caller ends the run before a sort step)
+    for (int32_t k = 0; k < n; ++k)
+        if (sort_due(h, t + (uint64_t)k)) { nsorts += 1; if (first_sort == n) first_sort = k; }
+    if (nsorts > 0 && h->Nc > kSmallSortCells) return MPCD_OK;
+    sa.sort_period = nsorts > 0 ? h->opt.sort_period : 0;
+    sa.first_sort = first_sort;
     const unsigned F = kSRD | kStream | kBin | fe | fixed_flag(h);
     if (h->opt.precision == MPCD_FP64) {
         const PassArgs<double> a = make_args<double>(h, pl);
@@ -594,6 +602,8 @@ int small_run(mpcd_t *h, int set, uint64_t t, int32_t n, unsigned fe, bool *done
     h->zeroed[0] = h->zeroed[1] = false;
     h->xi_valid[0] = h->xi_valid[1] = false;
     for (uint64_t u = t + (uint64_t)n - 1; u <= t + (uint64_t)n; ++u) { h->axis_valid[u & 1] = true; h->axis_step[u & 1] = u; }
+    h->sorts += (uint64_t)nsorts;
+    if (nsorts & 1) h->pcur ^= 1;                    // every sort inside the launch swapped the two sets of particle arrays
     return MPCD_OK;
 }
 
@@ -641,7 +651,6 @@ int do_sort(mpcd_t *h, int s, uint64_t t)
     return MPCD_OK;
 }
 
-inline bool sort_due(const mpcd_t *h, uint64_t t) { return h->opt.sort_period > 0 && (t % (uint64_t)h->opt.sort_period) == 0; }
 
 // bin + accumulate (+ axes) for step t as a standalone block; energy always accumulated here
 int bin_accumulate(mpcd_t *h, uint64_t t)
@@ -950,9 +959,9 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     // steady state, two launches per step: cell_prepare (zeroed set and axes of step t + 1), then collide(t) fused with
     // stream + bin + accumulate (t + 1)
     for (int32_t j = 1; j < nsteps; ++j) {
-        if (!at && !sort_pending && nsteps - j >= 2) {     // small systems: the run of steps up to the next sort in one cooperative launch
-            int32_t run = 1;
-            while (j + run < nsteps && !sort_due(h, t + (uint64_t)run)) ++run;
+        if (!at && nsteps - j >= 2 && (!sort_pending || h->Nc <= kSmallSortCells)) {   // small systems: a run of steps in one cooperative launch
+            int32_t run = 1;                               // up to the next sort step, or (few cells: the launch sorts itself) to the end of the call
+            while (j + run < nsteps && (h->Nc <= kSmallSortCells || !sort_due(h, t + (uint64_t)run))) ++run;
             bool done = false;
             if (run >= 2) { rc = small_run(h, set, t, run, fe, &done); if (rc) return rc; }
             if (done) {
