@@ -23,6 +23,8 @@
 //                    where they are accumulated (kBin) and where they are read (kSRD)
 //   kCoherent        the cell arrays read by kSRD were written earlier in the SAME launch (mpcd_small.cuh): plain loads ordered
 //                    by the grid barrier instead of the read-only (.nc) path, which promises data constant for the whole launch
+//   kCarry           the caller keeps the thread's particle in registers from one pass to the next (mpcd_small.cuh: the same
+//                    thread owns the same array slot in every phase between two sorts): no reload of what it has just stored
 //   kSortOut  a8     sort by cell on the way out: instead of in place, the particle is written
 //                    to slot cell_start[c] + (atomic cursor) of the duplicate arrays, c = its cell in the step
 //                    being collided; the separate read-and-scatter pass of the sort disappears
@@ -38,7 +40,7 @@
 
 namespace mpcdk {
 
-enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u, kEmbedded = 512u, kFixed = 1024u, kCoherent = 2048u };
+enum : unsigned { kSRD = 1u, kATApply = 2u, kStream = 4u, kBin = 8u, kEnergy = 16u, kATDraw = 32u, kSortOut = 64u, kThermo = 128u, kATStored = 256u, kEmbedded = 512u, kFixed = 1024u, kCoherent = 2048u, kCarry = 4096u };
 
 template <typename T> struct PassArgs {
     typename Vec4<T>::type *pos;
@@ -106,7 +108,8 @@ template <unsigned F> struct PassScratch {
 
 // The pass over one particle per thread (particle i = blockIdx.x * kPassThreads + threadIdx.x); `w` is the warp's scratch.
 template <typename T, unsigned F>
-__device__ __forceinline__ void pass_body(const PassArgs<T> &a, typename PassScratch<F>::type &w)
+__device__ __forceinline__ void pass_body(const PassArgs<T> &a, typename PassScratch<F>::type &w,
+                                          typename Vec4<T>::type *carry_p = nullptr, typename Vec4<T>::type *carry_v = nullptr, bool have = false)
 {
     using V4 = typename Vec4<T>::type;
     const int64_t i = (int64_t)blockIdx.x * kPassThreads + threadIdx.x;
@@ -117,8 +120,12 @@ __device__ __forceinline__ void pass_body(const PassArgs<T> &a, typename PassScr
     // Lanes past the end of the array (last block only) work on a copy of the last particle and simply do not store or
     // accumulate: no branch around the loads, the gather and the arithmetic, so the compiler schedules them as one block.
     const int64_t il = valid ? i : a.N - 1;
-    v = load4(a.vel + il);
-    if (F & (kStream | kBin)) p = load4(a.pos + il);
+    if ((F & kCarry) && have) {
+        v = *carry_v; p = *carry_p;
+    } else {
+        v = load4(a.vel + il);
+        if (F & (kStream | kBin)) p = load4(a.pos + il);
+    }
     if ((F & (kATDraw | kSortOut)) || ((F & kATApply) && !(F & kATStored))) tag = a.tag[il];
     int c = w_to_cell(v.w);                                      // cell of the last binning (the step being collided)
     int64_t o = i;                                               // where this particle is written
@@ -183,6 +190,7 @@ __device__ __forceinline__ void pass_body(const PassArgs<T> &a, typename PassScr
     }
     if ((F & (kSRD | kATApply | kBin)) && valid) store4(((F & kSortOut) ? a.vel_out : a.vel) + o, vs);
     if ((F & kSortOut) && valid) a.tag_out[o] = tag;
+    if (F & kCarry) { *carry_p = p; *carry_v = vs; }
     if (!valid) c = inactive;                                    // takes no part in the sums
     if constexpr ((F & kBin) && (F & kATDraw) && (F & kATStored))   // ONE sum per cell: sum(v) - sum(dv) is all eq. 4 needs; the stored dv is what is subtracted
         warp_cell_accumulate<T, true, (F & kEnergy) != 0, false, false, true>(a.acc, a.qacc, w, c, v.x, v.y, v.z, nullptr, 0.0, 0.0, 0.0, vs.x, vs.y, vs.z);

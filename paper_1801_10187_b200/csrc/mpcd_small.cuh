@@ -71,6 +71,8 @@ __global__ void __launch_bounds__(kPassThreads, 4) small_steps(PassArgs<T> a, co
     __shared__ typename PassScratch<F | kCoherent>::type ws[PassScratch<F | kCoherent>::count];
     const int64_t gtid = (int64_t)blockIdx.x * kPassThreads + threadIdx.x, gsize = (int64_t)gridDim.x * kPassThreads;
     int next_sort = s.sort_period > 0 ? s.first_sort : -1;
+    typename Vec4<T>::type carry_p = {}, carry_v = {};
+    bool have = false;
     for (int k = 0; k < s.nphases; ++k) {
         const uint64_t t = s.t0 + (uint64_t)k;
         const u32x4 b = draw(a.seed, t + 1, 0u, kDomShift);                   // a2: the grid shift of the step being binned
@@ -89,8 +91,10 @@ __global__ void __launch_bounds__(kPassThreads, 4) small_steps(PassArgs<T> a, co
             if (blockIdx.x == 0) small_scan_counts(a.sums, a.Nc, a.cursor, (F & kFixed) != 0);
             grid.sync();
             pass_body<T, F | kCoherent | kSortOut>(a, ws[threadIdx.x >> 5]);
+            have = false;                                // the slot holds another particle from now on
         } else {
-            pass_body<T, F | kCoherent>(a, ws[threadIdx.x >> 5]);
+            pass_body<T, F | kCoherent | kCarry>(a, ws[threadIdx.x >> 5], &carry_p, &carry_v, have);
+            have = true;                                 // this thread's particle stays in its registers for the next phase
         }
         double *ax = s.axis2[(t + 1) & 1], *z = s.acc3[(k + 2) % 3], *zq = s.qacc3[(k + 2) % 3];
         const bool more = k + 1 < s.nphases;
