@@ -158,7 +158,11 @@ int mpcd_sort(mpcd_t *h);
  * step t is fused with the streaming / binning / accumulation of step t + 1
  * (one pass over the particles per step), and on sort steps that pass also writes
  * the particles out in cell order; the result is the same as the unfused sequence
- * of calls up to fp64 summation order (exactly the same with opt.deterministic). */
+ * of calls up to fp64 summation order (exactly the same with opt.deterministic).
+ * A system small enough to sit on the device as one resident wave of thread blocks
+ * (plain SRD rule) runs its steps, sorts included, in one cooperative launch
+ * (DESIGN.md 5.4); the results are the same.  All work is enqueued on the handle's
+ * stream; the call does not synchronise. */
 int mpcd_step(mpcd_t *h, int32_t nsteps);
 
 /* Copies the particle state to caller-owned HOST buffers (any may be NULL):
