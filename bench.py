@@ -78,23 +78,24 @@ def csrc_hash(brick: int = 0) -> str:
 
 
 def ncu_traffic(workload: str, precision: str, brick: int):
-    """DRAM bytes per launch of the step kernel (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
-    `ncu --set full` summary profiles/ncu_traffic.csv (workload,precision,brick,bytes,csrc_hash,source).  A capture is
-    only quoted for the kernel sources it was taken on: returns (bytes or None, note)."""
+    """DRAM bytes per launch of the step kernel (dram__bytes_read.sum + dram__bytes_write.sum) and the busy fraction of its
+    actual limiter, the SM's LSU data pipe (l1tex__data_pipe_lsu_wavefronts, % of peak), from the committed `ncu --set full`
+    summary profiles/ncu_traffic.csv (workload,precision,brick,bytes,csrc_hash,lsu_pipe_pct,source).  A capture is only
+    quoted for the kernel sources it was taken on: returns (bytes or None, lsu pipe fraction or None, note)."""
     found = None
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
             for line in f:
                 w = [x.strip() for x in line.split(",")]
-                if len(w) >= 5 and w[0] == workload and w[1] == precision and w[2] == str(int(brick)):
-                    found = (float(w[3]), w[4])
+                if len(w) >= 6 and w[0] == workload and w[1] == precision and w[2] == str(int(brick)):
+                    found = (float(w[3]), w[4], float(w[5]) / 100.0)
     except Exception:
         pass
     if found is None:
-        return None, "no ncu capture committed for this workload"
+        return None, None, "no ncu capture committed for this workload"
     if found[1] != csrc_hash(brick):
-        return None, f"ncu capture is of kernel sources {found[1]}, the tree is {csrc_hash(brick)}: not quoted"
-    return found[0], f"ncu --set full capture of kernel sources {found[1]} (profiles/ncu_traffic.csv)"
+        return None, None, f"ncu capture is of kernel sources {found[1]}, the tree is {csrc_hash(brick)}: not quoted"
+    return found[0], found[2], f"ncu --set full capture of kernel sources {found[1]} (profiles/ncu_traffic.csv)"
 
 
 class ClockSampler:
@@ -344,11 +345,11 @@ def main():
     peak, peak_src = measured_peak()
     algo = algorithmic_bytes_per_particle(args.precision, M) * N
     achieved = algo / (fused_ms * 1e-3) / 1e9 if fused_ms > 0 else 0.0
-    traffic, traffic_note = ncu_traffic(args.config, args.precision, args.brick)
+    traffic, lsu_frac, traffic_note = ncu_traffic(args.config, args.precision, args.brick)
     kernel = "brick_pass" if args.brick else "particle_pass"
     roofline = {"bound": "hbm", "kernel": f"{kernel}<collide+stream+bin+accumulate> (steady-state fused step)",
                 "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "traffic_source": traffic_note, "algorithmic_bytes_per_launch": algo,
+                "traffic": traffic, "traffic_source": traffic_note, "lsu_data_pipe_busy_frac_ncu": lsu_frac, "algorithmic_bytes_per_launch": algo,
                 "kernel_ms": fused_ms, "kernel_share_of_step": fused_ms / (ms_max / timed),
                 "stage_ms_per_launch": {k: round(v[0], 4) for k, v in per_step_ms.items()},
                 "whole_step_frac": algo / (ms_max / timed * 1e-3) / 1e9 / peak}

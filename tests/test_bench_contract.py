@@ -49,6 +49,7 @@ def test_ncu_traffic_is_only_quoted_for_the_kernel_sources_it_was_taken_on():
     assert len(bench.csrc_hash()) == 16
     for row in open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")).read().splitlines()[1:]:
         w = [x.strip() for x in row.split(",")]
-        value, note = bench.ncu_traffic(w[0], w[1], int(w[2]))
-        assert (value is not None) == (w[4] == bench.csrc_hash(int(w[2]))), note
-    assert bench.ncu_traffic("C1", "mixed", 0) == (None, "no ncu capture committed for this workload")
+        value, lsu, note = bench.ncu_traffic(w[0], w[1], int(w[2]))
+        assert (value is not None) == (w[4] == bench.csrc_hash(int(w[2]))) == (lsu is not None), note
+        assert lsu is None or 0.0 < lsu <= 1.0
+    assert bench.ncu_traffic("C1", "mixed", 0) == (None, None, "no ncu capture committed for this workload")
