@@ -246,6 +246,47 @@ int mpcd_device_ptrs(mpcd_t *h, void **pos4, void **vel4, uint32_t **tag, int32_
  * mpcd_create when h == NULL).  Never NULL. */
 const char *mpcd_last_error(const mpcd_t *h);
 
+/*
+ * mpcd_cell_sums_static -- a3 + a4 without a handle and without any allocation: bins N particles into the shifted grid
+ * (A6, A8) and accumulates per cell the count, the sum of velocities and the kinetic energy in fp64
+ * (PAPER.md:118-124), exactly as mpcd_shift_and_bin does (same binning arithmetic, same warp-level reduction; the sums
+ * agree with mpcd_get_cells up to fp64 summation order, the counts exactly).
+ *
+ * It exists for callers that cannot obtain device memory at the point where they need the cell sums: code running
+ * beside an application that has given all device memory to another pool (a framework's caching allocator, an MPS
+ * client with a fixed memory limit), so that cudaMalloc fails; and code in a time-critical loop that cannot afford
+ * cudaMalloc / cudaFree because they may synchronise the device.  The call uses no cudaMalloc, no cudaFree, no
+ * allocator callback and no allocating library routine.  The per-cell accumulators it needs sit in a fixed array of
+ * MPCD_STATIC_MAX_CELLS * 40 bytes (1.25 MiB) inside the library, which each GPU holds from the time the library's
+ * device code is loaded onto it until the process exits.
+ *
+ * Arguments.  pos4, vel4: DEVICE, N x 4 of the native precision (float for MPCD_MIXED, double for MPCD_FP64), read
+ * only; the 4th components are ignored.  Positions must lie in [0, n[d] a) per axis (as for mpcd_set_state); a particle
+ * that does not is left out of every sum (nothing is written out of bounds).  n: HOST, cells per axis; a: cell edge;
+ * shift: HOST, the grid shift as applied, |shift[d]| < a (mixed model: pass the fp32 value, as mpcd_get_shift returns
+ * it); m: particle mass.  Outputs, DEVICE, caller-owned, any may be NULL: count[Nc] int32, sumv3[Nc * 3] and ke[Nc]
+ * double, Nc = n[0] n[1] n[2], cell index c = ix + n[0] (iy + n[1] iz), ke = m sum |v|^2 / 2.  N = 0 gives zeros.
+ * stream: cudaStream_t of the CURRENT device (NULL = legacy default stream); the work is enqueued there and the call
+ * does not synchronise.
+ *
+ * Errors: MPCD_EINVAL for Nc > MPCD_STATIC_MAX_CELLS (the message names the limit), N < 0 or >= 2^31, missing
+ * pointers, bad precision, a, m <= 0, |shift| >= a; MPCD_ECUDA for a runtime failure or no device.  The text is
+ * returned by mpcd_cell_sums_static_error() (per host thread; never NULL), not by mpcd_last_error.
+ *
+ * Sharing.  There is one scratch array per GPU and every call on that GPU uses it; it keeps the previous call's sums,
+ * so each call first clears the part it will use (on `stream`).  Two calls whose device work can overlap -- different
+ * streams, or different host threads -- race on it and give wrong sums: keep the calls of one GPU on one stream, or
+ * order them with events.
+ *
+ * First call.  The first call on each device (with that device current) looks up the array's device address
+ * (cudaGetSymbolAddress) and the SM count, under a lock, and keeps them; make that first call before any stream
+ * capture begins.
+ */
+#define MPCD_STATIC_MAX_CELLS 32768
+int mpcd_cell_sums_static(const void *pos4, const void *vel4, int64_t N, int32_t precision, const int32_t n[3], double a,
+                          const double shift[3], double m, int32_t *count, double *sumv3, double *ke, void *stream);
+const char *mpcd_cell_sums_static_error(void);
+
 /* Library identification: ABI version; build string (arch, compiler). */
 int mpcd_abi_version(void);
 const char *mpcd_build_info(void);

@@ -53,7 +53,9 @@ EXPORTS = [
     "mpcd_collide_srd", "mpcd_collide_at", "mpcd_sort", "mpcd_step", "mpcd_get_state", "mpcd_set_state",
     "mpcd_get_cells", "mpcd_get_shift", "mpcd_get_thermo", "mpcd_get_stats", "mpcd_device_ptrs", "mpcd_last_error",
     "mpcd_abi_version", "mpcd_build_info", "mpcd_test_philox", "mpcd_set_profiling", "mpcd_get_profile", "mpcd_get_xi", "mpcd_set_embedded", "mpcd_get_embedded",
+    "mpcd_cell_sums_static", "mpcd_cell_sums_static_error",
 ]
+STATIC_MAX_CELLS = 32768   # MPCD_STATIC_MAX_CELLS of include/mpcd.h
 PROF_KINDS = ("fused", "bin", "collide", "cells", "sort", "other", "fused_sort")
 
 _lib = None
@@ -93,8 +95,11 @@ def load_library():
     lib.mpcd_test_philox.argtypes = [vp, vp, vp, i64]
     lib.mpcd_set_profiling.argtypes = [vp, i32]
     lib.mpcd_get_profile.argtypes = [vp, P(dbl), P(u64)]
+    lib.mpcd_cell_sums_static.argtypes = [vp, vp, i64, i32, P(i32), dbl, P(dbl), dbl, vp, vp, vp, vp]
+    lib.mpcd_cell_sums_static_error.argtypes = []
+    lib.mpcd_cell_sums_static_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name not in ("mpcd_last_error", "mpcd_build_info"):
+        if name not in ("mpcd_last_error", "mpcd_build_info", "mpcd_cell_sums_static_error"):
             getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -286,6 +291,36 @@ class MPCD:
 
     def synchronize(self):
         self._stream.synchronize()
+
+
+def cell_sums_static(pos4, vel4, n, a, shift, m, count=None, sumv3=None, ke=None, stream=None):
+    """mpcd_cell_sums_static of include/mpcd.h: per-cell count, sum of velocities and kinetic energy of the particles in
+    the CUDA tensors pos4 / vel4 (N x 4, float32 = mixed model or float64), written into the caller's CUDA tensors
+    count (int32, Nc), sumv3 (float64, Nc x 3), ke (float64, Nc); any of the three may be None.
+
+    For callers that cannot allocate device memory where they need the sums (all of it belongs to another pool, or a
+    cudaMalloc's device synchronisation is not affordable): the library allocates nothing in this call, its accumulators
+    are a fixed 1.25 MiB array per GPU that holds at most STATIC_MAX_CELLS cells and that all calls on that GPU share.
+    Keep the calls of one GPU on one stream; the work is enqueued on `stream` (default: torch's current stream) and not
+    synchronised.  This wrapper allocates nothing on the device either: every tensor is the caller's."""
+    import torch
+    lib = load_library()
+    assert pos4.is_cuda and vel4.is_cuda and pos4.is_contiguous() and vel4.is_contiguous()
+    assert pos4.dtype == vel4.dtype and pos4.dtype in (torch.float32, torch.float64)
+    assert pos4.dim() == 2 and pos4.shape[1] == 4 and vel4.shape == pos4.shape
+    nn = (C.c_int32 * 3)(*[int(x) for x in n])
+    Nc = int(n[0]) * int(n[1]) * int(n[2])
+    for t, dt, numel in ((count, torch.int32, Nc), (sumv3, torch.float64, 3 * Nc), (ke, torch.float64, Nc)):
+        assert t is None or (t.is_cuda and t.is_contiguous() and t.dtype == dt and t.numel() == numel and t.device == pos4.device)
+    sh = (C.c_double * 3)(*[float(x) for x in shift])
+    st = stream if stream is not None else torch.cuda.current_stream(pos4.device)
+    dp = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+    with torch.cuda.device(pos4.device):
+        rc = lib.mpcd_cell_sums_static(dp(pos4) if pos4.shape[0] else None, dp(vel4) if pos4.shape[0] else None, pos4.shape[0],
+                                       MPCD_FP64 if pos4.dtype == torch.float64 else MPCD_MIXED, nn, float(a), sh, float(m),
+                                       dp(count), dp(sumv3), dp(ke), C.c_void_p(st.cuda_stream))
+    if rc != MPCD_OK:
+        raise MPCDError(rc, lib.mpcd_cell_sums_static_error().decode())
 
 
 def test_philox(ctr4, key2):

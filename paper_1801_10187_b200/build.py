@@ -1,6 +1,6 @@
 """Build the CUDA library (sm_100a) in-tree:  python -m paper_1801_10187_b200.build
 
-Produces paper_1801_10187_b200/libmpcd_b200.so from csrc/mpcd.cu with nvcc.  The .so is
+Produces paper_1801_10187_b200/libmpcd_b200.so from csrc/mpcd.cu and csrc/mpcd_static.cu with nvcc.  The .so is
 git-ignored but travels to the GPU box with the repo snapshot.
 """
 import os
@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmpcd_b200.so")
-SOURCES = ["mpcd.cu"]
+SOURCES = ["mpcd.cu", "mpcd_static.cu"]
 DEPS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh"))) + [os.path.join("..", "..", "include", "mpcd.h")]
 
 NVCC_FLAGS = [

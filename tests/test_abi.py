@@ -81,3 +81,28 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "oracle/" not in src.replace("shares nothing with oracle/", ""), f
+
+
+def test_static_cell_sums_validate_before_any_device_work(lib):
+    """mpcd_cell_sums_static (the no-allocation entry point): size and argument errors are reported on a box without a
+    GPU too, the limit is named in the message, and without a device a valid call fails loudly instead of computing."""
+    import torch
+    n_ok = (C.c_int32 * 3)(8, 8, 8)
+    n_big = (C.c_int32 * 3)(32, 32, 33)
+    n_huge = (C.c_int32 * 3)(2**31 - 1, 2**31 - 1, 2**31 - 1)
+    s = (C.c_double * 3)(0.1, -0.2, 0.3)
+    s_bad = (C.c_double * 3)(0.1, 1.0, 0.3)
+    f = lib.mpcd_cell_sums_static
+    err = lib.mpcd_cell_sums_static_error
+    assert f(None, None, 0, 0, n_big, 1.0, s, 1.0, None, None, None, None) == -1
+    assert b"32768" in err() and b"MPCD_STATIC_MAX_CELLS" in err()
+    assert f(None, None, 0, 0, n_huge, 1.0, s, 1.0, None, None, None, None) == -1
+    assert f(None, None, 5, 0, n_ok, 1.0, s, 1.0, None, None, None, None) == -1          # N > 0 without particle arrays
+    assert f(None, None, -1, 0, n_ok, 1.0, s, 1.0, None, None, None, None) == -1
+    assert f(None, None, 0, 2, n_ok, 1.0, s, 1.0, None, None, None, None) == -1          # precision
+    assert f(None, None, 0, 0, n_ok, 0.0, s, 1.0, None, None, None, None) == -1
+    assert f(None, None, 0, 0, n_ok, 1.0, s_bad, 1.0, None, None, None, None) == -1
+    assert f(None, None, 0, 0, None, 1.0, s, 1.0, None, None, None, None) == -1
+    if not torch.cuda.is_available():
+        assert f(None, None, 0, 0, n_ok, 1.0, s, 1.0, None, None, None, None) == -3      # MPCD_ECUDA
+        assert b"no CPU fallback" in err()
