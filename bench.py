@@ -15,7 +15,9 @@ Timing protocol ("whole multiples of the sort period so the sort i
 its period are PAPER.md:173, :177-179): the untimed warm-up runs at least --warmup steps and ends on a step
 with t % sort_period == 0; the timed region is ONE mpcd_step call of ceil(--steps / sort_period) * sort_period
 steps, so it always contains one sort per period whatever --steps says.  The line reports both counts
-(`steps` = timed, `steps_requested`, `warmup` = requested, `warmup_run`) and `check.sorts_in_timed_region`.
+(`steps` = as requested, `steps_timed` = what the timed call ran and what `ms_per_step` and `value` are computed over,
+`warmup` = requested, `warmup_run`) and `check.sorts_in_timed_region`.  The reference arm rounds the same way, so both
+arms time the same number of steps.
 
 Prints ONE JSON line (rank 0).  `value` = particle-steps/s with the state resident in HBM, timed
 with CUDA events on the library's stream around that mpcd_step call, max over ranks.  `e2e` = the same
@@ -53,6 +55,17 @@ UNIT = "particle-steps/s"
 def algorithmic_bytes_per_particle(precision: str, M: float) -> float:
     vec = 16 if precision == "mixed" else 32
     return 4 * vec + 80.0 / M
+
+
+# SURVEY.md 8d's headline model: two passes over the particles per step, B2 = 96 B (mixed) / 192 B (fp64) per particle-step
+# (read r, v; write r; write + read the cached cell index through v; read v; write v), + 4 B tag read for the AT rule.
+# The target sentence of BASELINE.md ("70 % of the HBM roofline") is N * B2 / t_step over 8 TB/s; the fused single-pass
+# kernel here moves less than B2, so this figure is a rate of useful work, not of bytes moved.
+def b2_bytes_per_particle(precision: str, rule: str) -> float:
+    return (96.0 if precision == "mixed" else 192.0) + (4.0 if rule == "at" else 0.0)
+
+
+NOMINAL_HBM_GBS = 8000.0   # BASELINE.json / SURVEY.md 8d "8 TB/s"
 
 
 def measured_peak():
@@ -218,6 +231,12 @@ def oracle_all_cores(cfg, precision, steps, warmup, n_sample):
     return sum(r[2] for r in res) / slowest, cores, res[0][2]
 
 
+def whole_periods(steps: int, period: int) -> int:
+    """max(steps, 1) rounded up to whole sort periods (period 0 = no sort: unchanged)."""
+    steps = max(int(steps), 1)
+    return -(-steps // period) * period if period > 0 else steps
+
+
 def sample_box(cfg, target_particles):
     """Cubic sub-box of about target_particles at the workload's density."""
     side = max(4, int(round((target_particles / cfg["M"]) ** (1.0 / 3.0))))
@@ -229,13 +248,17 @@ def run_reference(args, cfg, rank, world):
     if rank != 0:
         return 0
     n_sample = sample_box(cfg, args.ref_particles)
-    value, sec_per_step, Ns = oracle_sample(cfg, args.precision, args.steps, args.warmup, n_sample)
-    sample = f"{n_sample[0]}^3-cell sub-box of {args.config} at the same density ({Ns} particles), {args.steps} steps after {args.warmup} warm-up, sort every 25"
+    warm_run, timed = whole_periods(args.warmup, 25), whole_periods(args.steps, 25)      # as the GPU arm: both arms time the same number of steps
+    value, sec_per_step, Ns = oracle_sample(cfg, args.precision, timed, warm_run, n_sample)
+    sample = f"{n_sample[0]}^3-cell sub-box of {args.config} at the same density ({Ns} particles), {timed} steps after {warm_run} warm-up, sort every 25"
+    config = workload_config(args, cfg)
+    config.update({"sample": "each step advances a sub-box of the workload, not the whole box (tier framing: bounded sample)",
+                   "sample_cells": [int(x) for x in n_sample], "sample_particles": int(Ns)})
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "steps_timed": timed,
+        "warmup": args.warmup, "warmup_run": warm_run, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32 state / f64 cell sums + collision" if args.precision == "mixed" else "f64",
-        "data": "synthetic", "config": workload_config(args, cfg),
+        "data": "synthetic", "config": config,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -315,8 +338,7 @@ def main():
 
     # ---- device-resident throughput: whole sort periods, starting on a sort step ----
     P = max(args.sort_period, 0)
-    up = (lambda x: -(-x // P) * P) if P > 0 else (lambda x: x)
-    warm_run, timed = up(max(args.warmup, 1)), up(max(args.steps, 1))
+    warm_run, timed = whole_periods(args.warmup, P), whole_periods(args.steps, P)
     if warm_run < 3:
         raise SystemExit("bench.py: at least 3 warm-up steps are required (timing rules); give --warmup >= 3")
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -347,12 +369,19 @@ def main():
     achieved = algo / (fused_ms * 1e-3) / 1e9 if fused_ms > 0 else 0.0
     traffic, lsu_frac, traffic_note = ncu_traffic(args.config, args.precision, args.brick)
     kernel = "brick_pass" if args.brick else "particle_pass"
-    roofline = {"bound": "hbm", "kernel": f"{kernel}<collide+stream+bin+accumulate> (steady-state fused step)",
+    step_s = ms_max / timed * 1e-3
+    b2 = b2_bytes_per_particle(args.precision, cfg["rule"]) * N
+    lsu_note = f"ncu: l1tex__data_pipe_lsu_wavefronts {100 * lsu_frac:.0f} % busy" if lsu_frac else "no ncu capture of this workload on these kernel sources"
+    roofline = {"bound": "hbm", "limiter": f"HBM is the roofline the fraction is taken against; what the kernel actually saturates first is the SM's LSU data pipe ({lsu_note}; DESIGN.md 5.1)",
+                "kernel": f"{kernel}<collide+stream+bin+accumulate> (steady-state fused step)",
                 "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": traffic_note, "lsu_data_pipe_busy_frac_ncu": lsu_frac, "algorithmic_bytes_per_launch": algo,
                 "kernel_ms": fused_ms, "kernel_share_of_step": fused_ms / (ms_max / timed),
                 "stage_ms_per_launch": {k: round(v[0], 4) for k, v in per_step_ms.items()},
-                "whole_step_frac": algo / (ms_max / timed * 1e-3) / 1e9 / peak}
+                "whole_step_frac": algo / step_s / 1e9 / peak,
+                # the target's own figure: N * B2 / t_step, sort included, against 8 TB/s and against the measured copy peak
+                "b2_bytes_per_step": b2, "b2_gbs": b2 / step_s / 1e9, "b2_frac_of_8tbs": b2 / step_s / 1e9 / NOMINAL_HBM_GBS,
+                "b2_frac_of_measured": b2 / step_s / 1e9 / peak}
 
     # ---- end to end through the C ABI with host buffers ----
     e2e = None
@@ -407,7 +436,7 @@ def main():
 
     if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": timed, "steps_requested": args.steps,
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "steps_timed": timed,
             "warmup": args.warmup, "warmup_run": warm_run, "ms_per_step": ms_max / timed, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 state / f64 cell sums + collision" if args.precision == "mixed" else "f64",
             "data": "synthetic", "config": workload_config(args, cfg),

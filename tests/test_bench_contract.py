@@ -22,7 +22,11 @@ def test_reference_arm_prints_one_json_line_with_the_contract_keys():
     assert d["impl"] == "reference" and d["metric"] == "mpcd_particle_steps_per_s" and d["unit"] == "particle-steps/s"
     assert d["higher_is_better"] is True and d["scaling"] == "weak" and d["vs_baseline"] is None and d["data"] == "synthetic"
     assert d["steps"] == 2 and d["warmup"] == 3 and d["n_gpus"] == 1 and d["value"] > 0 and d["ms_per_step"] > 0
+    assert d["steps_timed"] == 25 and d["warmup_run"] == 25                      # whole sort periods, as the GPU arm times them
     assert d["config"]["workload"].startswith("C3") and "model" not in d["config"]
+    # the line says what ran: a sub-box of the workload, with its size
+    side = d["config"]["sample_cells"]
+    assert side[0] == side[1] == side[2] and d["config"]["sample_particles"] == side[0] ** 3 * 10 and "sub-box" in d["config"]["sample"]
     cb = d["cpu_baseline"]
     assert cb["kind"] == "oracle" and cb["cores"] == 1 and cb["value"] == d["value"] and "sub-box" in cb["sample"]
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}

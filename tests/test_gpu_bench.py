@@ -24,13 +24,17 @@ def test_gpu_arm_line_and_sort_aligned_timed_region():
     assert d["metric"] == "mpcd_particle_steps_per_s" and d["unit"] == "particle-steps/s" and d["higher_is_better"] is True
     assert d["n_gpus"] == 1 and d["scaling"] == "weak" and d["vs_baseline"] is None and d["data"] == "synthetic"
     # the driver's arguments cannot produce a sort-free window: 25 steps timed after 25, one sort inside
-    assert d["steps_requested"] == 20 and d["steps"] == 25 and d["warmup"] == 5 and d["warmup_run"] == 25
+    assert d["steps"] == 20 and d["steps_timed"] == 25 and d["warmup"] == 5 and d["warmup_run"] == 25
     assert d["check"]["sorts_in_timed_region"] == 1 and d["check"]["sort_period"] == 25
     assert abs(d["value"] - d["config"]["particles_per_gpu"] * 25 / (d["ms_per_step"] * 25e-3)) / d["value"] < 1e-9
     assert d["config"]["workload"].startswith("C2") and "model" not in d["config"]
     assert d["gpu_launches"] >= 25 and d["dtype"].startswith("f32")
     r = d["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["peak"] > 1000 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    # the target's own figure: N * 96 B per step (two-pass model B2) over the whole step, against 8 TB/s and the measured peak
+    assert r["b2_bytes_per_step"] == d["config"]["particles_per_gpu"] * 96 and "LSU" in r["limiter"]
+    assert abs(r["b2_frac_of_8tbs"] - r["b2_bytes_per_step"] / (d["ms_per_step"] * 1e-3) / 8e12) < 1e-9
+    assert abs(r["b2_frac_of_measured"] * r["peak"] - r["b2_frac_of_8tbs"] * 8000.0) < 1e-6
     assert r["kernel_ms"] > 0 and r["kernel_ms"] < d["ms_per_step"] and (r["traffic"] is None or r["traffic"] > 0) and r["traffic_source"]
     e = d["e2e"]
     assert e["unit"] == d["unit"] and e["value"] > 0 and e["value"] < d["value"]
@@ -45,7 +49,7 @@ def test_gpu_arm_line_and_sort_aligned_timed_region():
 
 def test_gpu_arm_rounds_longer_requests_up_and_honours_the_sort_period():
     d = _bench("--config", "C1", "--steps", "60", "--warmup", "30", "--sort-period", "10", "--no-e2e", "--no-cpu-baseline")
-    assert d["steps"] == 60 and d["warmup_run"] == 30 and d["check"]["sorts_in_timed_region"] == 6
+    assert d["steps"] == 60 and d["steps_timed"] == 60 and d["warmup_run"] == 30 and d["check"]["sorts_in_timed_region"] == 6
     d = _bench("--config", "C1", "--steps", "26", "--warmup", "3", "--no-e2e", "--no-cpu-baseline")
-    assert d["steps"] == 50 and d["warmup_run"] == 25 and d["check"]["sorts_in_timed_region"] == 2
+    assert d["steps"] == 26 and d["steps_timed"] == 50 and d["warmup_run"] == 25 and d["check"]["sorts_in_timed_region"] == 2
     assert d["e2e"] is None and d["cpu_baseline"] is None
