@@ -46,7 +46,9 @@ struct mpcd {
     double *axis[2] = {nullptr, nullptr};     // {nx, ny, nz, -} per cell
     // small systems (mpcd_small.cuh): a third accumulator set, allocated on first use; whether the cooperative kernel may be used
     double *acc_x = nullptr, *qacc_x = nullptr;
-    bool small_ok = true;
+    bool small_ok = true;          // cleared for good once a property that cannot change rules the cooperative path out
+    int small_capacity = -1;       // thread blocks of one resident wave of this handle's small_steps instantiation on this handle's device
+    std::vector<const void *> smem_configured;   // brick kernels whose dynamic shared memory opt-in has been set on this handle's device
     // embedded solute (NEXT-1; mpcd_embedded.cuh): beads in double, their per-cell sums by step parity
     int64_t emb_n = 0;
     int32_t emb_chain_len = 0, emb_nsub = 0;
@@ -338,10 +340,14 @@ BrickArgs brick_args(const mpcd_t *h, const PassPlan &pl)
 
 template <typename T, unsigned F> int launch_brick_t(mpcd_t *h, const PassArgs<T> &a, const BrickArgs &g)
 {
-    static bool configured = false;                  // dynamic shared memory above 48 KB is opt-in, once per instantiation
+    // dynamic shared memory above 48 KB is opt-in per kernel AND per device: remembered on the handle (which lives on one
+    // device and is used by one host thread at a time), not in a process-wide flag
+    const void *kern = reinterpret_cast<const void *>(brick_pass<T, F>);
+    bool configured = false;
+    for (const void *k : h->smem_configured) configured = configured || k == kern;
     if (!configured) {
         CUDA_TRY(h, cudaFuncSetAttribute(brick_pass<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BrickSmem<F>::bytes));
-        configured = true;
+        try { h->smem_configured.push_back(kern); } catch (...) { /* not remembered: set again at the next launch */ }
     }
     brick_pass<T, F><<<(unsigned)h->nbricks, kBrickThreads, BrickSmem<F>::bytes, h->stream>>>(a, g);
     return MPCD_OK;
@@ -529,32 +535,56 @@ inline bool sort_due(const mpcd_t *h, uint64_t t) { return h->opt.sort_period > 
 // Small systems: `n` consecutive fused steps (collide t .. t + n - 1, none of them a sort step) as ONE cooperative launch
 // (mpcd_small.cuh).  Returns MPCD_OK with *done = false when the system is not eligible (too large for one resident wave,
 // another rule, thermostat, beads, brick order, profiling): the caller then takes the ordinary per-step path.
-template <typename T, unsigned F> int small_launch_t(mpcd_t *h, const PassArgs<T> &a, const SmallArgs &sa, bool *done)
+// The instantiation of small_steps a handle uses (its precision, energy option and accumulation mode never change), or
+// nullptr when there is none for these flags.
+const void *small_kernel(const mpcd_t *h, unsigned F)
 {
-    static int capacity = -1;                        // blocks of one resident wave, per instantiation
-    if (capacity < 0) {
-        int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, small_steps<T, F>, kPassThreads, 0) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
-        capacity = per_sm * h->num_sms;
+#define SMALL(T, f) reinterpret_cast<const void *>(small_steps<T, (f)>)
+    if (h->opt.precision == MPCD_FP64) {
+        switch (F) {
+            case kSRD | kStream | kBin: return SMALL(double, kSRD | kStream | kBin);
+            case kSRD | kStream | kBin | kEnergy: return SMALL(double, kSRD | kStream | kBin | kEnergy);
+            default: return nullptr;
+        }
     }
-    const unsigned grid = grid_for(h->N, kPassThreads);
-    if ((int64_t)grid > (int64_t)capacity) return MPCD_OK;
-    void *args[2] = {const_cast<PassArgs<T> *>(&a), const_cast<SmallArgs *>(&sa)};
-    if (cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(small_steps<T, F>), dim3(grid), dim3(kPassThreads), args, 0, h->stream) != cudaSuccess) {
-        cudaGetLastError();                          // no cooperative launch on this device / context: never try again
+    switch (F) {
+        case kSRD | kStream | kBin: return SMALL(float, kSRD | kStream | kBin);
+        case kSRD | kStream | kBin | kEnergy: return SMALL(float, kSRD | kStream | kBin | kEnergy);
+        case kSRD | kStream | kBin | kFixed: return SMALL(float, kSRD | kStream | kBin | kFixed);
+        case kSRD | kStream | kBin | kEnergy | kFixed: return SMALL(float, kSRD | kStream | kBin | kEnergy | kFixed);
+        default: return nullptr;
+    }
+#undef SMALL
+}
+
+// Whether the cooperative path can ever serve this handle, from what cannot change after mpcd_create.  Cheap, and evaluated
+// before mpcd_step looks for a run of steps: a handle that fails it never pays for the search.
+inline bool small_possible(mpcd_t *h)
+{
+    if (!h->small_ok) return false;
+    if (h->opt.rule != MPCD_SRD || thermostatted(h) || h->grid.on
+        || h->N > (int64_t)h->num_sms * 16 * kPassThreads                                 // cannot be one resident wave whatever the kernel
+        || h->Nc > 4 * (int64_t)grid_for(h->N, kPassThreads) * kPassThreads)              // a dilute box: the cell side (an fp64 sincos per cell) would dominate the phase
         h->small_ok = false;
-        return MPCD_OK;
-    }
-    *done = true;
-    return MPCD_OK;
+    return h->small_ok;
 }
 
 int small_run(mpcd_t *h, int set, uint64_t t, int32_t n, unsigned fe, bool *done)
 {
     *done = false;
-    if (!h->small_ok || h->profiling || h->debug_sync || h->opt.rule != MPCD_SRD || thermostatted(h) || embedded(h) || h->grid.on) return MPCD_OK;
-    if (h->N > (int64_t)h->num_sms * 16 * kPassThreads) return MPCD_OK;              // cannot be one resident wave whatever the kernel
-    if (h->Nc > 4 * (int64_t)grid_for(h->N, kPassThreads) * kPassThreads) return MPCD_OK;   // a dilute box: the cell side (an fp64 sincos per cell) would dominate the phase
+    if (!small_possible(h) || h->profiling || h->debug_sync || embedded(h)) return MPCD_OK;
+    // one resident wave of THIS handle's kernel on THIS handle's device: asked once, before anything is allocated or zeroed;
+    // N and the occupancy are fixed, so a handle that does not fit never comes back here
+    const unsigned F = kSRD | kStream | kBin | fe | fixed_flag(h);
+    const void *kern = small_kernel(h, F);
+    if (!kern) { h->small_ok = false; return MPCD_OK; }
+    if (h->small_capacity < 0) {
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kPassThreads, 0) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+        h->small_capacity = per_sm * h->num_sms;
+    }
+    const unsigned grid = grid_for(h->N, kPassThreads);
+    if ((int64_t)grid > (int64_t)h->small_capacity) { h->small_ok = false; return MPCD_OK; }
     if (!h->acc_x) {
         int rc = dev_alloc_t(h, &h->acc_x, (size_t)h->Nc * 4);
         if (!rc) rc = dev_alloc_t(h, &h->qacc_x, (size_t)h->Nc);
@@ -580,22 +610,15 @@ int small_run(mpcd_t *h, int set, uint64_t t, int32_t n, unsigned fe, bool *done
     if (nsorts > 0 && h->Nc > kSmallSortCells) return MPCD_OK;
     sa.sort_period = nsorts > 0 ? h->opt.sort_period : 0;
     sa.first_sort = first_sort;
-    const unsigned F = kSRD | kStream | kBin | fe | fixed_flag(h);
-    if (h->opt.precision == MPCD_FP64) {
-        const PassArgs<double> a = make_args<double>(h, pl);
-        if (F & kEnergy) rc = small_launch_t<double, kSRD | kStream | kBin | kEnergy>(h, a, sa, done);
-        else rc = small_launch_t<double, kSRD | kStream | kBin>(h, a, sa, done);
-    } else {
-        const PassArgs<float> a = make_args<float>(h, pl);
-        switch (F) {
-            case kSRD | kStream | kBin: rc = small_launch_t<float, kSRD | kStream | kBin>(h, a, sa, done); break;
-            case kSRD | kStream | kBin | kEnergy: rc = small_launch_t<float, kSRD | kStream | kBin | kEnergy>(h, a, sa, done); break;
-            case kSRD | kStream | kBin | kFixed: rc = small_launch_t<float, kSRD | kStream | kBin | kFixed>(h, a, sa, done); break;
-            case kSRD | kStream | kBin | kEnergy | kFixed: rc = small_launch_t<float, kSRD | kStream | kBin | kEnergy | kFixed>(h, a, sa, done); break;
-            default: break;
-        }
+    const PassArgs<double> a64 = make_args<double>(h, pl);
+    const PassArgs<float> a32 = make_args<float>(h, pl);
+    void *args[2] = {h->opt.precision == MPCD_FP64 ? (void *)&a64 : (void *)&a32, &sa};
+    if (cudaLaunchCooperativeKernel(kern, dim3(grid), dim3(kPassThreads), args, 0, h->stream) != cudaSuccess) {
+        cudaGetLastError();                          // no cooperative launch on this device / context: never try again
+        h->small_ok = false;
+        return MPCD_OK;
     }
-    if (rc || !*done) return rc;
+    *done = true;
     LAUNCH_CHECK(h);
     // cell-array state after n phases: the sums of step t + n are complete in set (t + n) & 1, the axes of steps t + n and
     // t + n - 1 in their parities; every other set is dirty
@@ -959,9 +982,12 @@ int mpcd_step(mpcd_t *h, int32_t nsteps)
     // steady state, two launches per step: cell_prepare (zeroed set and axes of step t + 1), then collide(t) fused with
     // stream + bin + accumulate (t + 1)
     for (int32_t j = 1; j < nsteps; ++j) {
-        if (!at && nsteps - j >= 2 && (!sort_pending || h->Nc <= kSmallSortCells)) {   // small systems: a run of steps in one cooperative launch
-            int32_t run = 1;                               // up to the next sort step, or (few cells: the launch sorts itself) to the end of the call
-            while (j + run < nsteps && (h->Nc <= kSmallSortCells || !sort_due(h, t + (uint64_t)run))) ++run;
+        if (!at && nsteps - j >= 2 && (!sort_pending || h->Nc <= kSmallSortCells) && small_possible(h)) {   // small systems: a run of steps in one cooperative launch
+            int32_t run = nsteps - j;                      // to the end of the call (few cells: the launch sorts itself) ...
+            if (h->Nc > kSmallSortCells && h->opt.sort_period > 0) {   // ... or up to the next sort step, t + r with r >= 1
+                const int64_t r = (int64_t)h->opt.sort_period - (int64_t)(t % (uint64_t)h->opt.sort_period);
+                if (r < (int64_t)run) run = (int32_t)r;
+            }
             bool done = false;
             if (run >= 2) { rc = small_run(h, set, t, run, fe, &done); if (rc) return rc; }
             if (done) {
