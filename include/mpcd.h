@@ -87,7 +87,15 @@ typedef struct mpcd_options {
                               brick[0] x brick[1] x brick[2] cells (mpcd_stats.brick; compile-time), bricks x-fastest over
                               ceil(n_d / brick[d]) per axis, cells x-fastest inside a brick -- and mpcd_step runs its steady-state kernel
                               with one thread block per brick and the cell side of the step in shared memory.  The
-                              order inside the sort is free (A20): results are the same up to fp64 summation order.
+                              order inside the sort is free (A20): results are the same up to fp64 summation order, with one
+                              qualification.  The block-local partial sums are fixed-point: with unit = the power of two >=
+                              sqrt(kT/m) of mpcd_create, a velocity component is rounded to 2^-49 unit and |v|^2 to 2^-44 unit^2
+                              before it is added (exact for fp32 state; for MPCD_FP64 about 16x coarser than a double at
+                              |v| ~ unit: cell means move by <= 2^-50 unit, velocities after a collision by < 1e-13 unit, a
+                              thermostat factor by ~1e-14 relative -- inside the 1e-12 tolerance, but not "summation order"
+                              only).  A particle with any |v_d| >= 8 unit does not fit that format and takes the per-particle
+                              route (direct fp64 atomics): correct, but slow if it is most of them, e.g. a state loaded with
+                              mpcd_set_state at > 60x the kT given to mpcd_create or in a bulk drift above 8 unit.
                               0 (default): ascending cell index and the warp-level kernel (the faster of the two on the north-star workload,
                               DESIGN.md 5.1) */
     void *stream;          /* cudaStream_t the library enqueues on; NULL = the legacy default stream */

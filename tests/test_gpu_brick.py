@@ -170,3 +170,33 @@ def test_brick_kernel_keeps_the_invariants_over_many_sort_periods():
     assert np.array_equal(np.sort(s["tag"]), tag)
     assert np.all((s["pos"][:, :3] >= 0) & (s["pos"][:, :3] < 64.0))
     g.close()
+
+
+@pytest.mark.parametrize("kT_state", [1.0, 150.0])
+def test_fp64_brick_sums_stay_within_their_stated_quantisation(kT_state):
+    """include/mpcd.h, opt.brick: in the fp64 model the brick kernel's block-local sums round a velocity component to
+    2^-49 unit (unit = the power of two >= sqrt(kT/m) of the handle) -- coarser than the per-particle kernel's fp64 atomics,
+    so "same up to summation order" does not quite hold.  The stated bound: a cell mean moves by <= 2^-50 unit, a velocity
+    after the collision by < 1e-13 unit.  Checked brick = 1 against brick = 0 on the same fluid over one sort and two
+    brick launches.  Second case: a state at 150x the handle's kT, where most particles have a component above 8 unit,
+    do not fit the fixed-point headroom and take the direct fp64 route: same agreement (scaled by |v| ~ 12 unit)."""
+    from paper_1801_10187_b200 import MPCD
+    n, M = (16, 12, 10), 10
+    pos, vel, tag = synth.solvent(n, M, seed=23, dtype=np.float64, kT=kT_state)
+    if kT_state > 64.0:
+        assert np.mean(np.max(np.abs(vel[:, :3]), axis=1) >= 8.0) > 0.5
+    out = []
+    for brick in (True, False):
+        g = MPCD([float(x) for x in n], pos.shape[0], kT=1.0, seed=23, precision="fp64", init_state=False, brick=brick, sort_period=25,
+                 dt=0.1 if kT_state == 1.0 else 0.02)
+        g.set_state(pos, vel, tag)
+        g.step(3)                     # step 0 sorts; the collisions of steps 0 and 1 run in the step kernel under test
+        assert (g.stats()["brick"][0] > 0) == brick
+        s = g.get_state()
+        o = np.argsort(s["tag"], kind="stable")
+        out.append((s["pos"][o][:, :3], s["vel"][o][:, :3], s["cell"][o]))
+        g.close()
+    scale = math.sqrt(kT_state)
+    assert np.array_equal(out[0][2], out[1][2])
+    assert np.max(np.abs(out[0][1] - out[1][1])) < 1e-13 * scale * 3       # three collisions
+    assert np.max(np.abs(out[0][0] - out[1][0])) < 1e-13 * scale
