@@ -277,7 +277,7 @@ def workload_config(args, cfg):
     return {"workload": f"{args.config}: MPCD-{cfg['rule'].upper()} solvent{solute}, {n[0]}x{n[1]}x{n[2]} cells (a=1), density {cfg['M']}, "
                         f"{n[0] * n[1] * n[2] * cfg['M']} particles, alpha=130deg, dt=0.1, random grid shift, sort every 25, {args.precision} precision",
             "particles_per_gpu": n[0] * n[1] * n[2] * cfg["M"], "cells_per_gpu": n[0] * n[1] * n[2],
-            "precision": args.precision, "cell_energy": bool(args.cell_energy),
+            "precision": args.precision, "cell_energy": bool(args.cell_energy), "thermostat": bool(args.thermostat),
             "parallelism": f"replicas x{args.gpus} (one GPU per box, no data-path collective)",
             "l2_policy": "working set (6.4 GB mixed / 11.5 GB fp64 at C3) >> 126 MB L2; no flush needed"}
 
@@ -293,6 +293,7 @@ def main():
     ap.add_argument("--cell-energy", type=int, default=1)
     ap.add_argument("--sort-period", type=int, default=25)
     ap.add_argument("--brick", type=int, default=0, help="1: brick-major sort order + the brick-tiled step kernel")
+    ap.add_argument("--thermostat", type=int, default=0, help="1: Maxwell-Boltzmann cell thermostat on (SRD rule; for profiling cell_thermostat and the kThermo kernels)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -329,7 +330,7 @@ def main():
     pos, vel, tag = synth.solvent(n, M, seed=seed, dtype=dtype)
     N = pos.shape[0]
     sim = MPCD([float(x) for x in n], N, seed=seed, precision=args.precision, rule=cfg["rule"], sort_period=args.sort_period,
-               cell_energy=bool(args.cell_energy), init_state=False, brick=bool(args.brick), device=f"cuda:{local_rank}")
+               cell_energy=bool(args.cell_energy), init_state=False, brick=bool(args.brick), thermostat=bool(args.thermostat), device=f"cuda:{local_rank}")
     sim.set_state(pos, vel, tag)
     if "chains" in cfg:
         ch = cfg["chains"]

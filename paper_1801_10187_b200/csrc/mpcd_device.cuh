@@ -57,6 +57,33 @@ __device__ __forceinline__ void draw_axis(uint64_t seed, uint64_t step, uint32_t
     nx = rho * c; ny = rho * s; nz = z;
 }
 
+// The same axis formed per PARTICLE in registers instead of being gathered from the per-cell array ("or
+// recomputed per particle in a6"; probe MPCD_AXIS_REG): it depends on (seed, step, cell) only.  The fp64
+// model evaluates draw_axis itself (the same bits as the stored axis).  The mixed model evaluates the transcendental part in
+// fp32 (reading A13b): z, 1 - z and 1 + z exactly in double from the 53-bit uniform, rho = sqrtf of their product (relative
+// error 1e-7, also at the poles), the azimuth from the top 32 of its 53 bits (angle error < 1.5e-9) split into 24 exact
+// bits for sincospif + a first-order rotation; then the vector is renormalised in double (|n|^2 - 1 ~ 1e-20, so the
+// rotation conserves the cell's energy as exactly as with the stored axis).  The direction differs from the fp64 axis
+// by <= ~1.5e-7, i.e. velocities by <= 2 |v - u| 1.5e-7 < 1e-5 sigma.
+template <typename T>
+__device__ __forceinline__ void axis_in_registers(uint64_t seed, uint64_t step, uint32_t cell, double &nx, double &ny, double &nz)
+{
+    if (sizeof(T) == 8) { draw_axis(seed, step, cell, nx, ny, nz); return; }
+    const u32x4 b = draw(seed, step, cell, kDomAxis);
+    const double u = u01_53(b.x, b.y);
+    const double z = 2.0 * u - 1.0;
+    const float rho = sqrtf((float)((2.0 - 2.0 * u) * (2.0 * u)));                 // (1 - z)(1 + z), the factors exact
+    const float hi = (float)(b.w >> 8) * 1.1920928955078125e-7f;                  // 2 U2 = b.w 2^-31 = hi + lo (units of pi): (b.w >> 8) 2^-23 + (b.w & 255) 2^-31
+    const float lo = (float)(b.w & 255u) * 4.656612873077392578125e-10f;
+    float sh, ch;
+    sincospif(hi, &sh, &ch);
+    const float d = 3.14159265358979323846f * lo;
+    const double x = (double)(rho * fmaf(-d, sh, ch)), y = (double)(rho * fmaf(d, ch, sh));
+    const double e = fma(x, x, fma(y, y, fma(z, z, -1.0)));                        // |n|^2 - 1, ~2e-7
+    const double inv = fma(e, fma(e, 0.375, -0.5), 1.0);                           // (1 + e)^(-1/2) to O(e^3)
+    nx = x * inv; ny = y * inv; nz = z * inv;
+}
+
 // Three Gaussians of unit variance by Box-Muller from one Philox block keyed by the particle
 // tag (A17, A18); the fourth is discarded.
 __device__ __forceinline__ void gauss3_from_block(const u32x4 b, double &g0, double &g1, double &g2)

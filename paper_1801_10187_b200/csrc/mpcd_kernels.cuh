@@ -69,6 +69,12 @@ template <typename T> struct PassArgs {
     uint64_t seed, step_collide, step_bin;
 };
 
+// Probe: 1 = the SRD collision of the plain rule forms the cell's axis in registers instead of gathering it.
+#ifndef MPCD_AXIS_REG
+#define MPCD_AXIS_REG 0
+#endif
+constexpr bool kAxisReg = MPCD_AXIS_REG != 0;
+
 #ifndef MPCD_PASS_THREADS
 #define MPCD_PASS_THREADS 128
 #endif
@@ -133,7 +139,13 @@ __device__ __forceinline__ void pass_body(const PassArgs<T> &a, typename PassScr
     if (F & kSRD) {
         {
             f64x4 s = (F & kCoherent) ? ld256(a.sums + 4 * (size_t)c) : ld256_nc(a.sums + 4 * (size_t)c);   // Alg. 1 lines 2-4: the cell's sums and axis, one sector each
-            const f64x4 n = (F & kCoherent) ? ld256(a.axis + 4 * (size_t)c) : ld256_nc(a.axis + 4 * (size_t)c);
+            f64x4 n;
+            if constexpr (kAxisReg && !(F & (kThermo | kFixed | kCoherent))) {   // probe: no second gathered sector (xi rides in the axis sector; the deterministic mode keeps every kernel on the stored bits)
+                axis_in_registers<T>(a.seed, a.step_collide, (uint32_t)c, n.x, n.y, n.z);
+                n.w = 1.0;
+            } else {
+                n = (F & kCoherent) ? ld256(a.axis + 4 * (size_t)c) : ld256_nc(a.axis + 4 * (size_t)c);
+            }
             if (F & kFixed) { s.x = acc_value(s.x, true); s.y = acc_value(s.y, true); s.z = acc_value(s.z, true); s.w = acc_count(s.w, true); }
             double ux, uy, uz;
             if (F & kEmbedded) {
