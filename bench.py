@@ -20,7 +20,8 @@ steps, so it always contains one sort per period whatever --steps says.  The lin
 arms time the same number of steps.
 
 Prints ONE JSON line (rank 0).  `value` = particle-steps/s with the state resident in HBM, timed
-with CUDA events on the library's stream around that mpcd_step call, max over ranks.  `e2e` = the same
+with CUDA events on the library's stream around that mpcd_step call, max over ranks (workloads below 10 M particles: >= 5 such windows,
+about one second in all, the median window reported -- `windows`).  `e2e` = the same
 metric through the C ABI with HOST buffers: every step copies the state from pinned host memory
 (mpcd_set_state), steps, and copies it back (mpcd_get_state).  `roofline` = algorithmic bytes of
 the steady-state fused kernel / its live-measured duration, against the measured HBM copy peak.
@@ -294,6 +295,11 @@ def main():
     ap.add_argument("--sort-period", type=int, default=25)
     ap.add_argument("--brick", type=int, default=0, help="1: brick-major sort order + the brick-tiled step kernel")
     ap.add_argument("--thermostat", type=int, default=0, help="1: Maxwell-Boltzmann cell thermostat on (SRD rule; for profiling cell_thermostat and the kThermo kernels)")
+    ap.add_argument("--min-ms", type=float, default=None,
+                    help="repeat the timed window until the windows add up to this many ms (then at least 5 windows, the median reported); "
+                         "default: 1000 for workloads below 10 M particles, whose single window is too short for the 10 ms clock sampler, "
+                         "0 (one window of exactly the whole sort periods asked for, as in rounds 1-2) for the large ones")
+    ap.add_argument("--max-windows", type=int, default=400)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -302,6 +308,8 @@ def main():
     ap.add_argument("--ref-particles", type=int, default=2_000_000, help="--impl reference sample size per step")
     args = ap.parse_args()
     cfg = synth.CONFIGS[args.config]
+    if args.min_ms is None:
+        args.min_ms = 1000.0 if cfg["n"][0] * cfg["n"][1] * cfg["n"][2] * cfg["M"] < 10_000_000 else 0.0
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -354,6 +362,21 @@ def main():
         barrier()
         ms = ev0.elapsed_time(ev1)
         st1 = sim.stats()
+        # SURVEY.md 8d "median of >= 5 windows", for the small configurations (--min-ms): the same timed call repeated (every window
+        # again whole sort periods starting on a sort step) until the windows add up to about a second, so that a workload whose
+        # window is a few ms is timed over a stretch in which the 10 ms clock sampler sees the GPU under load.  All ranks run the
+        # same number of windows.  The large configurations keep ONE window of exactly the steps asked for.
+        _, ms_first = replicas.whole_job_throughput(float(N) * timed, ms, dist if world > 1 else None, dev)
+        windows = [ms]
+        nwin = min(max(int(math.ceil(args.min_ms / max(ms_first, 1e-3))), 5), args.max_windows) if args.min_ms > 0 else 1
+        for _ in range(nwin - 1):
+            barrier()
+            ev0.record()
+            sim.step(timed)
+            ev1.record()
+            barrier()
+            windows.append(ev0.elapsed_time(ev1))
+        ms = float(np.median(windows))
         # ---- per-kernel durations, live, CUDA events on the library's stream, over one more whole sort period ----
         sim.set_profiling(True)
         sim.step(max(P, 1) + 1)
@@ -439,6 +462,8 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "steps_timed": timed,
             "warmup": args.warmup, "warmup_run": warm_run, "ms_per_step": ms_max / timed, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "windows": {"count": len(windows), "steps_each": timed, "ms_min": float(min(windows)), "ms_median": float(np.median(windows)), "ms_max": float(max(windows)),
+                        "note": "value and ms_per_step are over the median window of this rank, max over ranks; gpu_launches counts one window"},
             "dtype": "f32 state / f64 cell sums + collision" if args.precision == "mixed" else "f64",
             "data": "synthetic", "config": workload_config(args, cfg),
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": int(launches),

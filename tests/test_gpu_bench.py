@@ -26,6 +26,9 @@ def test_gpu_arm_line_and_sort_aligned_timed_region():
     # the driver's arguments cannot produce a sort-free window: 25 steps timed after 25, one sort inside
     assert d["steps"] == 20 and d["steps_timed"] == 25 and d["warmup"] == 5 and d["warmup_run"] == 25
     assert d["check"]["sorts_in_timed_region"] == 1 and d["check"]["sort_period"] == 25
+    w = d["windows"]                                       # >= 5 windows of 25 steps each, the median one reported
+    assert w["count"] >= 5 and w["steps_each"] == 25 and w["ms_min"] <= w["ms_median"] <= w["ms_max"]
+    assert abs(w["ms_median"] / 25 - d["ms_per_step"]) < 1e-9
     assert abs(d["value"] - d["config"]["particles_per_gpu"] * 25 / (d["ms_per_step"] * 25e-3)) / d["value"] < 1e-9
     assert d["config"]["workload"].startswith("C2") and "model" not in d["config"]
     assert d["gpu_launches"] >= 25 and d["dtype"].startswith("f32")
