@@ -57,3 +57,18 @@ def test_ncu_traffic_is_only_quoted_for_the_kernel_sources_it_was_taken_on():
         assert (value is not None) == (w[4] == bench.csrc_hash(int(w[2]))) == (lsu is not None), note
         assert lsu is None or 0.0 < lsu <= 1.0
     assert bench.ncu_traffic("C1", "mixed", 0) == (None, None, "no ncu capture committed for this workload")
+
+
+def test_whole_sort_periods_and_the_b2_byte_model():
+    """Both arms round --steps / --warmup up to whole sort periods; the target's byte model is SURVEY.md 8d's B2."""
+    sys.path.insert(0, ROOT)
+    import bench
+    assert [bench.whole_periods(k, 25) for k in (0, 1, 20, 25, 26, 100)] == [25, 25, 25, 25, 50, 100]
+    assert bench.whole_periods(7, 0) == 7 and bench.whole_periods(0, 0) == 1 and bench.whole_periods(60, 10) == 60
+    assert bench.b2_bytes_per_particle("mixed", "srd") == 96 and bench.b2_bytes_per_particle("fp64", "srd") == 192
+    assert bench.b2_bytes_per_particle("mixed", "at") == 100
+    # C3 mixed: N * B2 = 7.68 GB, so 70 % of 8 TB/s is 1.37 ms per step = 58 G particle-steps/s (SURVEY.md 8d)
+    N = 80_000_000
+    t = N * bench.b2_bytes_per_particle("mixed", "srd") / (0.70 * bench.NOMINAL_HBM_GBS * 1e9)
+    assert abs(t * 1e3 - 1.371) < 1e-3 and abs(N / t / 1e9 - 58.3) < 0.1
+    assert bench.algorithmic_bytes_per_particle("mixed", 10) == 72 and bench.algorithmic_bytes_per_particle("fp64", 10) == 136
